@@ -1,0 +1,186 @@
+/* tpcclus.h — C-ABI boundary of the B200-native TPC cluster finder.
+ *
+ * What the library computes
+ * -------------------------
+ * Cluster finding on zero-suppressed, continuous-readout TPC digits of one
+ * time-frame fragment: charge-map fill, 3x3 local-maximum peak finding,
+ * monotone-descent 5x5 cluster assembly, charge-weighted centroid and width,
+ * ordered stream compaction.  The paper (PAPER.md:58 §3.1, :116 §4, :142 §4.2)
+ * states the problem — ZS digits of a time frame in, reconstructed TPC clusters
+ * out, the whole TF processed on one GPU with memory reused across steps — and
+ * names no algorithm; the five steps come from BASELINE.json:north_star and the
+ * exact definitions D1..D12 from SURVEY.md §8(c) (restated in DESIGN.md §2).
+ *
+ * Conventions
+ * -----------
+ *  - "host" / "device" is stated for every pointer.  No torch types, no C++
+ *    types, no exceptions cross this boundary.
+ *  - Every function returns an int status: 0 = TPCCLUS_OK, negative = error.
+ *  - A context is not thread-safe; distinct contexts are independent.
+ *  - Nothing is allocated inside tpcclus_run ("GPU memory reuse
+ *    across processing steps became essential"); all scratch is sized in
+ *    tpcclus_create from the geometry.
+ *  - Determinism: the output bytes depend only on the SET of digits, the
+ *    geometry and the core range — not on digit order inside a sector slice,
+ *    launch configuration or run number.
+ */
+#ifndef TPCCLUS_H
+#define TPCCLUS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------ */
+#define TPCCLUS_OK             0
+#define TPCCLUS_ERR_INVALID   -1  /* null / misaligned pointer, core range larger than max_core_bins,
+                                     core outside the TF, offsets not monotone, n > max_digits       */
+#define TPCCLUS_ERR_GEOMETRY  -2  /* npads out of 1..248, zero sizes, halo_bins in 1..4, tf > 65536   */
+#define TPCCLUS_ERR_CAPACITY  -3  /* more clusters than out_capacity: the first out_capacity records
+                                     are valid and ordered, stats.n_clusters is the number required
+                                     (hit count fluctuates -> "safety margin")         */
+#define TPCCLUS_ERR_DIGIT     -4  /* strict mode only: some digit was out of range / NaN / zero       */
+#define TPCCLUS_ERR_CUDA      -5  /* stats.cuda_error holds the cudaError_t                           */
+#define TPCCLUS_ERR_NOMEM     -6  /* device or pinned-host allocation failed in create                */
+
+/* ---- cluster flag bits ---------------------------- */
+#define TPCCLUS_FLAG_EDGE_PAD   0x01u /* peak pad < 2 or >= npads[row]-2                      */
+#define TPCCLUS_FLAG_EDGE_TIME  0x02u /* peak time < 2 or >= tf_time_bins-2 (true TF ends)    */
+#define TPCCLUS_FLAG_SATURATED  0x04u /* peak or a member has q16 == 16368 (1023 ADC)         */
+#define TPCCLUS_FLAG_SPLIT      0x08u /* some member cell is shared with another peak (S>=2)  */
+
+/* ---- geometry option bits ---------------------------------------------- */
+#define TPCCLUS_OPT_STRICT_DIGITS 0x0001u /* an invalid digit makes the run fail with ERR_DIGIT
+                                             instead of being dropped and counted             */
+#define TPCCLUS_OPT_HOST_STAGING  0x0002u /* allocate the device staging buffers that
+                                             tpcclus_run_host / tpcclus_run_tf_host need
+                                             (2 x max_digits digits + 2 x max_clusters records) */
+
+#define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
+#define TPCCLUS_MAX_NPADS  248u
+#define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
+
+/* One zero-suppressed digit, 8 bytes (BASELINE.json:configs[0]: "uint8 row, uint8 pad,
+ * uint16 time, float32 charge").  time is the GLOBAL time bin inside the TF.  The sector is
+ * not in the record: digits arrive grouped per sector (see sector_offsets below). */
+typedef struct {
+  uint8_t  row;
+  uint8_t  pad;
+  uint16_t time;
+  float    charge;   /* ADC counts; quantised by the library to q16 = clamp(rint(16*charge),0,16368) (D1) */
+} tpcclus_digit;
+
+/* One cluster, 32 bytes, one per peak (D8, D10).  Integer fields are bit-exact by contract;
+ * the five floats are the real-number definitions of D8 evaluated from exact integer moments. */
+typedef struct {
+  uint8_t  sector, row, pad, flags; /* peak cell + TPCCLUS_FLAG_* bits                       */
+  uint32_t time;                    /* peak cell, global TF time bin                          */
+  uint16_t qmax_q16;                /* peak charge in 1/16 ADC                                */
+  uint16_t ncells;                  /* 1..25 cells contributing (peak + members)              */
+  float    qtot;                    /* ADC: sum of shared charge, W / (16*2520)               */
+  float    dpad, dtime;             /* centroid minus peak cell, each in (-2, 2)              */
+  float    sigma_pad, sigma_time;   /* sqrt of the charge-weighted central second moment      */
+} tpcclus_cluster;
+
+/* Detector shape and scratch sizing; read once by tpcclus_create (npads is copied). */
+typedef struct {
+  uint32_t n_sectors, n_rows;       /* 36, 152 in the configs; any >= 1                        */
+  const uint16_t* npads;            /* HOST array [n_rows], each 1..TPCCLUS_MAX_NPADS          */
+  uint32_t tf_time_bins;            /* whole-TF length, e.g. 57024; 1..65536 (u16 digit time)  */
+  uint32_t max_core_bins;           /* largest fragment core passed to run, e.g. 4096          */
+  uint32_t halo_bins;               /* digits loaded each side of the core: 0 (single
+                                       fragment) or >= TPCCLUS_MIN_HALO; 8 in configs[3]       */
+  uint16_t peak_min_q16;            /* theta_peak >= 1 (D11); 64 = 4 ADC is the default used
+                                       by the tests and the bench                              */
+  uint16_t options;                 /* TPCCLUS_OPT_* bits                                      */
+  uint64_t max_digits;              /* largest n passed to run                                 */
+  uint64_t max_clusters;            /* sizing of the host-staging cluster buffers only         */
+} tpcclus_geometry;
+
+typedef struct {
+  uint64_t n_digits_in;             /* n of the run                                            */
+  uint64_t n_digits_dropped;        /* invalid digits (row/pad/time out of range, NaN, q16==0) */
+  uint64_t n_clusters;              /* clusters REQUIRED (may exceed out_capacity)             */
+  int32_t  status;                  /* TPCCLUS_OK or the error of the run                      */
+  int32_t  cuda_error;              /* cudaError_t when status == TPCCLUS_ERR_CUDA             */
+} tpcclus_run_stats;
+
+/* One fragment of a time frame held in HOST memory, for tpcclus_run_tf_host. */
+typedef struct {
+  const tpcclus_digit* h_digits;    /* HOST, n digits grouped per sector                       */
+  uint64_t n;
+  const uint64_t* h_sector_offsets; /* HOST [n_sectors+1]                                      */
+  uint32_t t_core_begin, t_core_end;
+} tpcclus_fragment;
+
+typedef struct tpcclus_ctx tpcclus_ctx; /* opaque; owns all device scratch */
+
+/* Create a context on CUDA device `cuda_device`.  Allocates the charge map
+ * (n_sectors x sum(pitch(npads)) x (max_core_bins + 2*halo_bins) uint16), the per-(sector,row)
+ * TMA descriptors, tile-scan state and a pinned status block.
+ * Errors: ERR_INVALID (null), ERR_GEOMETRY, ERR_NOMEM, ERR_CUDA (no device / wrong arch). */
+int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out);
+
+/* Enqueue one fragment on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
+ * stream).  Asynchronous: returns after the launches; call tpcclus_result for the outcome.
+ *   d_digits          DEVICE, n records, 8-byte aligned, read-only, owned by the caller and
+ *                     must stay valid until the run has finished.
+ *   h_sector_offsets  HOST [n_sectors+1], monotone, off[0]==0, off[n_sectors]==n; digits of
+ *                     sector s are d_digits[off[s] .. off[s+1]), in ANY order.  Read during
+ *                     the call, not retained.
+ *   t_core_begin/end  core [b,e) in global time bins, 0 <= b < e <= tf_time_bins,
+ *                     e-b <= max_core_bins.  Digits with time in [b-halo, e+halo) (clipped to
+ *                     the TF) are loaded, all others are dropped and counted; exactly the
+ *                     clusters whose PEAK time lies in [b,e) are emitted (D9,
+ *                     BASELINE.json:configs[3]).
+ *   d_out             DEVICE, out_capacity records, 16-byte aligned, owned by the caller.
+ *                     Record k is the k-th peak in ascending (sector,row,time,pad) (D10).
+ * At most one digit per cell is a precondition (D2); the result for duplicate cells is
+ * unspecified but memory-safe.  One run in flight per context.
+ * Errors (immediate): ERR_INVALID, ERR_CUDA.  Deferred to tpcclus_result: ERR_CAPACITY,
+ * ERR_DIGIT, ERR_CUDA. */
+int tpcclus_run(tpcclus_ctx* ctx, const tpcclus_digit* d_digits, uint64_t n,
+                const uint64_t* h_sector_offsets,
+                uint32_t t_core_begin, uint32_t t_core_end,
+                tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
+
+/* Wait for the run enqueued by tpcclus_run and report it.  Returns stats->status. */
+int tpcclus_result(tpcclus_ctx* ctx, tpcclus_run_stats* stats);
+
+/* Same operation with HOST buffers (pageable or pinned): copies the digits host->device,
+ * runs, copies min(n_clusters, out_capacity) records device->host, synchronises.  Needs
+ * TPCCLUS_OPT_HOST_STAGING; n <= max_digits; out_capacity is clipped to max_clusters. */
+int tpcclus_run_host(tpcclus_ctx* ctx, const tpcclus_digit* h_digits, uint64_t n,
+                     const uint64_t* h_sector_offsets,
+                     uint32_t t_core_begin, uint32_t t_core_end,
+                     tpcclus_cluster* h_out, uint64_t out_capacity, tpcclus_run_stats* stats);
+
+/* A whole time frame from HOST memory, fragment by fragment ("streamed through device
+ * memory", BASELINE.json:configs[3]): the host->device copy of fragment k+1
+ * and the device->host copy of fragment k-1 overlap the kernels of fragment k (two staging
+ * slots, three streams).  Fragment f writes its records to h_out + sum of the counts of the
+ * fragments before it (D10: a TF's list is the concatenation of its fragments' lists);
+ * stats[f] reports fragment f.  Returns the first non-OK fragment status, else OK.
+ * h_out has out_capacity records in total. */
+int tpcclus_run_tf_host(tpcclus_ctx* ctx, const tpcclus_fragment* frags, uint32_t n_frags,
+                        tpcclus_cluster* h_out, uint64_t out_capacity,
+                        tpcclus_run_stats* stats /* HOST [n_frags] */);
+
+/* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
+uint64_t tpcclus_launch_count(const tpcclus_ctx* ctx);
+
+/* Bytes of device memory the context owns (charge map + scratch + staging). */
+uint64_t tpcclus_device_bytes(const tpcclus_ctx* ctx);
+
+/* Free everything.  NULL is allowed. */
+void tpcclus_destroy(tpcclus_ctx* ctx);
+
+/* Static string for a status code. */
+const char* tpcclus_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCCLUS_H */

@@ -1,0 +1,165 @@
+"""ORACLE binding — test infrastructure, not product.
+
+Loads ``oracle/libtpc_oracle.so`` (plain single-threaded C++, ``tpc_oracle.cpp``) through
+ctypes.  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` leg may import this module.  It imports nothing from
+``paper_2412_13755_b200`` and the product imports nothing from here.
+
+The record dtypes below restate BASELINE.json:configs[0] (8-byte digit) and SURVEY.md §8(b)
+(32-byte cluster) on their own.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_LIB = os.path.join(_HERE, "libtpc_oracle.so")
+
+DIGIT_DTYPE = np.dtype(
+    [("row", "u1"), ("pad", "u1"), ("time", "<u2"), ("charge", "<f4")], align=False
+)
+CLUSTER_DTYPE = np.dtype(
+    [
+        ("sector", "u1"), ("row", "u1"), ("pad", "u1"), ("flags", "u1"),
+        ("time", "<u4"),
+        ("qmax_q16", "<u2"), ("ncells", "<u2"),
+        ("qtot", "<f4"), ("dpad", "<f4"), ("dtime", "<f4"),
+        ("sigma_pad", "<f4"), ("sigma_time", "<f4"),
+    ],
+    align=False,
+)
+assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
+
+FLAG_EDGE_PAD, FLAG_EDGE_TIME, FLAG_SATURATED, FLAG_SPLIT = 1, 2, 4, 8
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [
+        ("n_sectors", ctypes.c_uint32), ("n_rows", ctypes.c_uint32),
+        ("npads", ctypes.POINTER(ctypes.c_uint16)),
+        ("tf_time_bins", ctypes.c_uint32), ("halo_bins", ctypes.c_uint32),
+        ("peak_min_q16", ctypes.c_uint16), ("reserved", ctypes.c_uint16),
+    ]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [
+        ("n_digits_in", ctypes.c_uint64), ("n_digits_dropped", ctypes.c_uint64),
+        ("n_duplicates", ctypes.c_uint64), ("n_clusters", ctypes.c_uint64),
+        ("sum_q16_loaded", ctypes.c_uint64), ("sum_W", ctypes.c_uint64),
+    ]
+
+
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (no CUDA, no other dependency)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp%d" % os.getpid()
+        subprocess.check_call(
+            ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall", "-Wextra", _SRC, "-o", tmp]
+        )
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    with _lock:
+        if _lib is None:
+            lib = ctypes.CDLL(build())
+            lib.tpc_oracle_run.restype = ctypes.c_int
+            lib.tpc_oracle_run.argtypes = [
+                ctypes.POINTER(_Params), ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p,
+                ctypes.c_uint32, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_uint64,
+                ctypes.POINTER(_Stats),
+            ]
+            lib.tpc_oracle_quantise.restype = ctypes.c_uint16
+            lib.tpc_oracle_quantise.argtypes = [ctypes.c_float]
+            lib.tpc_oracle_peak_flags.restype = ctypes.c_int64
+            lib.tpc_oracle_peak_flags.argtypes = [
+                ctypes.POINTER(_Params), ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p,
+                ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
+                ctypes.c_void_p, ctypes.c_void_p,
+            ]
+            _lib = lib
+    return _lib
+
+
+def _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16):
+    npads = np.ascontiguousarray(npads, dtype=np.uint16)
+    p = _Params()
+    p.n_sectors = int(n_sectors)
+    p.n_rows = int(npads.shape[0])
+    p.npads = npads.ctypes.data_as(ctypes.POINTER(ctypes.c_uint16))
+    p.tf_time_bins = int(tf_time_bins)
+    p.halo_bins = int(halo_bins)
+    p.peak_min_q16 = int(peak_min_q16)
+    return p, npads
+
+
+def quantise(charge: float) -> int:
+    """D1 for one value."""
+    return int(_load().tpc_oracle_quantise(ctypes.c_float(charge)))
+
+
+def run(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, t_core_begin=0,
+        t_core_end=None, halo_bins=0, peak_min_q16=64, capacity=None):
+    """Cluster one fragment.  Returns (clusters[CLUSTER_DTYPE], stats dict).
+
+    digits: array of DIGIT_DTYPE grouped per sector by sector_offsets[n_sectors+1].
+    """
+    lib = _load()
+    digits = np.ascontiguousarray(digits, dtype=DIGIT_DTYPE)
+    offs = np.ascontiguousarray(sector_offsets, dtype=np.uint64)
+    assert offs.shape[0] == n_sectors + 1
+    if t_core_end is None:
+        t_core_end = tf_time_bins
+    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16)
+    st = _Stats()
+    if capacity is None:
+        # count first, then allocate exactly
+        rc = lib.tpc_oracle_run(ctypes.byref(prm), digits.ctypes.data, digits.shape[0],
+                                offs.ctypes.data, t_core_begin, t_core_end, None, 0,
+                                ctypes.byref(st))
+        if rc != 0:
+            raise ValueError("tpc_oracle_run: bad arguments")
+        capacity = int(st.n_clusters)
+    out = np.zeros(int(capacity), dtype=CLUSTER_DTYPE)
+    rc = lib.tpc_oracle_run(ctypes.byref(prm), digits.ctypes.data, digits.shape[0],
+                            offs.ctypes.data, t_core_begin, t_core_end,
+                            out.ctypes.data if capacity else None, capacity, ctypes.byref(st))
+    if rc != 0:
+        raise ValueError("tpc_oracle_run: bad arguments")
+    del keep
+    stats = {k: int(getattr(st, k)) for k, _ in _Stats._fields_}
+    return out[: min(int(st.n_clusters), int(capacity))], stats
+
+
+def peak_flags(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, sector, row,
+               t_core_begin=0, t_core_end=None, halo_bins=0, peak_min_q16=64):
+    """D4 flags and the q16 map of one (sector,row): two arrays [ntime_loaded, npads[row]]."""
+    lib = _load()
+    digits = np.ascontiguousarray(digits, dtype=DIGIT_DTYPE)
+    offs = np.ascontiguousarray(sector_offsets, dtype=np.uint64)
+    if t_core_end is None:
+        t_core_end = tf_time_bins
+    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16)
+    lo = max(0, t_core_begin - halo_bins)
+    hi = min(tf_time_bins, t_core_end + halo_bins)
+    w = int(keep[row])
+    flags = np.zeros((hi - lo, w), dtype=np.uint8)
+    q = np.zeros((hi - lo, w), dtype=np.uint16)
+    n = lib.tpc_oracle_peak_flags(ctypes.byref(prm), digits.ctypes.data, digits.shape[0],
+                                  offs.ctypes.data, t_core_begin, t_core_end, sector, row,
+                                  flags.ctypes.data, q.ctypes.data)
+    assert n == hi - lo
+    return flags, q
