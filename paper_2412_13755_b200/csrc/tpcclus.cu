@@ -1,0 +1,409 @@
+// tpcclus.cu — C-ABI of include/tpcclus.h on top of the sm_100a kernels in tpcclus_kernels.cuh.
+//
+// Host logic only: argument checks, geometry tables, TMA descriptors, launches, the
+// host-staging pipeline.  Every step of the path runs in the kernels.  The CUDA driver API is
+// reached through cudaGetDriverEntryPoint (cuTensorMapEncodeTiled), so the library links
+// against the static CUDA runtime only and loads on a box without a GPU driver (where
+// tpcclus_create then fails loudly with TPCCLUS_ERR_CUDA — there is no CPU fallback).
+#include "../../include/tpcclus.h"
+#include "tpcclus_kernels.cuh"
+
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace tpcclus;
+
+static_assert(sizeof(tpcclus_digit) == 8, "digit is 8 bytes");
+static_assert(sizeof(tpcclus_cluster) == 32 && sizeof(tpcclus_cluster) == sizeof(ClusterRec), "cluster is 32 bytes");
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct tpcclus_ctx {
+  tpcclus_geometry g{};
+  std::vector<uint16_t> npads;
+  std::vector<RowInfo> rows;
+  int device = 0;
+  uint32_t H = 0;                 // map rows per (sector,row): max_core_bins + 2*halo_bins
+  uint64_t sec_elems = 0;         // map elements per sector
+  uint32_t max_tiles = 0;
+  uint32_t tile_bytes_max = 0, bm_words = 0, smem_bytes = 0;
+  int cluster_grid = 0;           // persistent grid of k_cluster
+  int n_sm = 0;
+  uint32_t epoch = 0;
+  uint64_t launches = 0;
+  uint64_t dev_bytes = 0;
+  // device
+  uint16_t* d_map = nullptr;
+  RowInfo* d_rows = nullptr;
+  CUtensorMap* d_tmaps = nullptr;
+  unsigned long long* d_tile_state = nullptr;
+  DevStatus* d_status = nullptr;
+  // pinned host
+  DevStatus* h_status = nullptr;
+  // last run
+  cudaStream_t last_stream = nullptr;
+  bool run_pending = false;
+  uint64_t last_n = 0, last_cap = 0;
+  int sticky = TPCCLUS_OK;
+  int sticky_cuda = 0;
+  // host staging (TPCCLUS_OPT_HOST_STAGING)
+  tpcclus_digit* d_stage_digits[2] = {nullptr, nullptr};
+  tpcclus_cluster* d_stage_out[2] = {nullptr, nullptr};
+  cudaStream_t s_h2d = nullptr, s_run = nullptr, s_d2h = nullptr;
+  cudaEvent_t ev_h2d[2] = {nullptr, nullptr}, ev_run[2] = {nullptr, nullptr}, ev_d2h[2] = {nullptr, nullptr};
+};
+
+namespace {
+
+inline uint32_t roundup(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
+
+int cuda_fail(tpcclus_ctx* c, cudaError_t e) {
+  if (c) { c->sticky = TPCCLUS_ERR_CUDA; c->sticky_cuda = int(e); }
+  return TPCCLUS_ERR_CUDA;
+}
+
+#define CK(ctx, call)                                  \
+  do {                                                 \
+    cudaError_t e__ = (call);                          \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__); \
+  } while (0)
+
+template <typename T>
+int dev_alloc(tpcclus_ctx* c, T** p, uint64_t bytes) {
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes ? bytes : 16);
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return TPCCLUS_ERR_NOMEM; }
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  c->dev_bytes += bytes;
+  return TPCCLUS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tpcclus_strerror(int code) {
+  switch (code) {
+    case TPCCLUS_OK: return "ok";
+    case TPCCLUS_ERR_INVALID: return "invalid argument";
+    case TPCCLUS_ERR_GEOMETRY: return "invalid geometry";
+    case TPCCLUS_ERR_CAPACITY: return "cluster output capacity exceeded";
+    case TPCCLUS_ERR_DIGIT: return "invalid digit in strict mode";
+    case TPCCLUS_ERR_CUDA: return "CUDA error";
+    case TPCCLUS_ERR_NOMEM: return "out of memory";
+    default: return "unknown status";
+  }
+}
+
+void tpcclus_destroy(tpcclus_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->device);
+  if (c->s_run) cudaStreamSynchronize(c->s_run);
+  if (c->last_stream || c->run_pending) cudaStreamSynchronize(c->last_stream);
+  cudaFree(c->d_map); cudaFree(c->d_rows); cudaFree(c->d_tmaps); cudaFree(c->d_tile_state); cudaFree(c->d_status);
+  if (c->h_status) cudaFreeHost(c->h_status);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(c->d_stage_digits[i]); cudaFree(c->d_stage_out[i]);
+    if (c->ev_h2d[i]) cudaEventDestroy(c->ev_h2d[i]);
+    if (c->ev_run[i]) cudaEventDestroy(c->ev_run[i]);
+    if (c->ev_d2h[i]) cudaEventDestroy(c->ev_d2h[i]);
+  }
+  if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
+  if (c->s_run) cudaStreamDestroy(c->s_run);
+  if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
+  delete c;
+}
+
+int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out) {
+  if (!g || !out || !g->npads) return TPCCLUS_ERR_INVALID;
+  *out = nullptr;
+  if (g->n_sectors < 1 || g->n_sectors > (uint32_t)kMaxSectors || g->n_rows < 1 || g->n_rows > 256 ||
+      g->tf_time_bins < 1 || g->tf_time_bins > 65536 || g->max_core_bins < 1 ||
+      g->max_core_bins > g->tf_time_bins || (g->halo_bins >= 1 && g->halo_bins < TPCCLUS_MIN_HALO) ||
+      g->halo_bins > 4096 || g->peak_min_q16 < 1 || g->peak_min_q16 > TPCCLUS_QMAX_Q16)
+    return TPCCLUS_ERR_GEOMETRY;
+  for (uint32_t r = 0; r < g->n_rows; ++r)
+    if (g->npads[r] < 1 || g->npads[r] > TPCCLUS_MAX_NPADS) return TPCCLUS_ERR_GEOMETRY;
+
+  tpcclus_ctx* c = new (std::nothrow) tpcclus_ctx();
+  if (!c) return TPCCLUS_ERR_NOMEM;
+  c->g = *g;
+  c->npads.assign(g->npads, g->npads + g->n_rows);
+  c->g.npads = c->npads.data();
+  c->device = cuda_device;
+
+  auto fail = [&](int rc) { tpcclus_destroy(c); return rc; };
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
+  if (prop.major < 10) return fail(TPCCLUS_ERR_CUDA);       // TMA + sm_100a code only; no fallback
+  c->n_sm = prop.multiProcessorCount;
+
+  // geometry tables
+  c->H = g->max_core_bins + 2 * g->halo_bins;
+  c->rows.resize(g->n_rows);
+  uint64_t off = 0;
+  uint32_t max_boxw = 0, max_npads = 0;
+  for (uint32_t r = 0; r < g->n_rows; ++r) {
+    RowInfo& ri = c->rows[r];
+    ri.npads = c->npads[r];
+    ri.pitch = uint16_t(roundup(ri.npads, 8));
+    ri.boxw = uint16_t(roundup(ri.npads + 2 * kPadHalo, 8));
+    ri.nwords = uint16_t((ri.npads + 1) / 2);
+    if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
+    ri.map_off = uint32_t(off);
+    off += uint64_t(c->H) * ri.pitch;
+    max_boxw = std::max<uint32_t>(max_boxw, ri.boxw);
+    max_npads = std::max<uint32_t>(max_npads, ri.npads);
+  }
+  c->sec_elems = off;
+  c->tile_bytes_max = roundup(uint32_t(kBoxH) * max_boxw * 2u, 128);
+  c->bm_words = (max_npads + 8 + 31) / 32 + 1;
+  const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * ((g->max_core_bins + kTileT - 1) / kTileT);
+  if (tiles > 0x7FFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
+  c->max_tiles = uint32_t(tiles);
+  c->smem_bytes = kStages * c->tile_bytes_max + kBoxH * c->bm_words * 4 + (kTileT + 1) * 4 + kListCap * 4 +
+                  256 * sizeof(RowInfo) + kStages * 8 + kStages * 4 + 16 * 4 + 128;
+
+  int rc;
+  const uint64_t map_bytes = uint64_t(g->n_sectors) * c->sec_elems * 2;
+  if ((rc = dev_alloc(c, &c->d_map, map_bytes)) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_rows, g->n_rows * sizeof(RowInfo))) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_tmaps, uint64_t(g->n_sectors) * g->n_rows * sizeof(CUtensorMap))) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_tile_state, uint64_t(c->max_tiles) * 8)) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_status, sizeof(DevStatus))) != TPCCLUS_OK) return fail(rc);
+  if (cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DevStatus)) != cudaSuccess) return fail(TPCCLUS_ERR_NOMEM);
+  if (cudaMemcpy(c->d_rows, c->rows.data(), g->n_rows * sizeof(RowInfo), cudaMemcpyHostToDevice) != cudaSuccess ||
+      cudaMemset(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8) != cudaSuccess ||
+      cudaMemset(c->d_status, 0, sizeof(DevStatus)) != cudaSuccess)
+    return fail(TPCCLUS_ERR_CUDA);
+
+  // one 2-D TMA descriptor per (sector,row): dims {npads, H}, row stride pitch*2 bytes,
+  // box {boxw, kBoxH}; out-of-range box elements are zero-filled (D2)
+  {
+    PFN_encodeTiled encode = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    void* fn = nullptr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || !fn)
+      return fail(TPCCLUS_ERR_CUDA);
+    encode = reinterpret_cast<PFN_encodeTiled>(fn);
+    std::vector<CUtensorMap> maps(size_t(g->n_sectors) * g->n_rows);
+    for (uint32_t s = 0; s < g->n_sectors; ++s)
+      for (uint32_t r = 0; r < g->n_rows; ++r) {
+        const RowInfo& ri = c->rows[r];
+        cuuint64_t gdim[2] = {ri.npads, c->H};
+        cuuint64_t gstr[1] = {cuuint64_t(ri.pitch) * 2};
+        cuuint32_t box[2] = {ri.boxw, cuuint32_t(kBoxH)};
+        cuuint32_t estr[2] = {1, 1};
+        void* base = c->d_map + uint64_t(s) * c->sec_elems + ri.map_off;
+        CUresult cr = encode(&maps[size_t(s) * g->n_rows + r], CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, base, gdim, gstr,
+                             box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cr != CUDA_SUCCESS) return fail(TPCCLUS_ERR_CUDA);
+      }
+    if (cudaMemcpy(c->d_tmaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess)
+      return fail(TPCCLUS_ERR_CUDA);
+  }
+
+  if (cudaFuncSetAttribute(k_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, int(c->smem_bytes)) != cudaSuccess)
+    return fail(TPCCLUS_ERR_CUDA);
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cluster, kThreads, c->smem_bytes) != cudaSuccess || occ < 1)
+    return fail(TPCCLUS_ERR_CUDA);
+  c->cluster_grid = occ * c->n_sm;
+
+  if (g->options & TPCCLUS_OPT_HOST_STAGING) {
+    for (int i = 0; i < 2; ++i) {
+      if ((rc = dev_alloc(c, &c->d_stage_digits[i], g->max_digits * sizeof(tpcclus_digit))) != TPCCLUS_OK) return fail(rc);
+      if ((rc = dev_alloc(c, &c->d_stage_out[i], g->max_clusters * sizeof(tpcclus_cluster))) != TPCCLUS_OK) return fail(rc);
+      if (cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&c->ev_run[i], cudaEventDisableTiming) != cudaSuccess ||
+          cudaEventCreateWithFlags(&c->ev_d2h[i], cudaEventDisableTiming) != cudaSuccess)
+        return fail(TPCCLUS_ERR_CUDA);
+    }
+    if (cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->s_run, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking) != cudaSuccess)
+      return fail(TPCCLUS_ERR_CUDA);
+  }
+  if (cudaDeviceSynchronize() != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
+  *out = c;
+  return TPCCLUS_OK;
+}
+
+int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const uint64_t* h_off,
+                uint32_t b, uint32_t e, tpcclus_cluster* d_out, uint64_t cap, void* cuda_stream) {
+  if (!c || !h_off || (n && !d_digits) || (cap && !d_out)) return TPCCLUS_ERR_INVALID;
+  const tpcclus_geometry& g = c->g;
+  if (!(b < e) || e > g.tf_time_bins || e - b > g.max_core_bins || n > g.max_digits) return TPCCLUS_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_digits) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return TPCCLUS_ERR_INVALID;
+  if (h_off[0] != 0 || h_off[g.n_sectors] != n) return TPCCLUS_ERR_INVALID;
+  for (uint32_t s = 0; s < g.n_sectors; ++s)
+    if (h_off[s + 1] < h_off[s]) return TPCCLUS_ERR_INVALID;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  CK(c, cudaSetDevice(c->device));
+
+  const int32_t origin = int32_t(b) - int32_t(g.halo_bins);
+  const uint32_t tiles_per_row = (e - b + kTileT - 1) / kTileT;
+  const uint32_t n_tiles = g.n_sectors * g.n_rows * tiles_per_row;
+  // rows of the map that a TMA box of this run can touch (rows >= H are zero-filled by TMA)
+  const uint32_t rows_used = std::min<uint32_t>(c->H, tiles_per_row * kTileT + g.halo_bins + kReach);
+  c->epoch = (c->epoch + 1) & 0x3FFFFFFFu;
+  if (c->epoch == 0) {   // wrapped: stale words could alias, so wipe them once
+    CK(c, cudaMemsetAsync(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8, st));
+    c->epoch = 1;
+  }
+
+  // S0: clear
+  {
+    uint32_t max_pitch = 0;
+    for (const RowInfo& ri : c->rows) max_pitch = std::max<uint32_t>(max_pitch, ri.pitch);
+    const uint64_t span16 = (uint64_t(rows_used) * max_pitch) >> 3;
+    const uint32_t chunks = uint32_t(std::min<uint64_t>(std::max<uint64_t>((span16 + 256 * 8 - 1) / (256 * 8), 1), 65535));
+    dim3 grid(g.n_sectors * g.n_rows, chunks);
+    k_clear<<<grid, 256, 0, st>>>(c->d_map, c->d_rows, g.n_rows, c->sec_elems, rows_used, c->d_status);
+    c->launches++;
+  }
+  // S1: scatter
+  if (n) {
+    ScatterParams sp;
+    sp.n = n;
+    sp.sec_elems = c->sec_elems;
+    sp.t_origin = origin;
+    sp.t_lo = std::max<int32_t>(0, origin);
+    sp.t_hi = int32_t(std::min<uint64_t>(g.tf_time_bins, uint64_t(e) + g.halo_bins));
+    sp.n_sectors = g.n_sectors;
+    sp.n_rows = g.n_rows;
+    std::memcpy(sp.off, h_off, (g.n_sectors + 1) * sizeof(uint64_t));
+    const uint64_t pairs = (n + 1) / 2;
+    const uint32_t blocks = uint32_t(std::min<uint64_t>((pairs + 255) / 256, uint64_t(c->n_sm) * 16));
+    k_scatter<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), sp, c->d_rows, c->d_map, c->d_status);
+    c->launches++;
+  }
+  // S2..S7: fused tile kernel
+  {
+    ClusterParams cp;
+    cp.tmaps = c->d_tmaps;
+    cp.rows = c->d_rows;
+    cp.tile_state = c->d_tile_state;
+    cp.status = c->d_status;
+    cp.out = d_out;
+    cp.out_capacity = cap;
+    cp.n_sectors = g.n_sectors;
+    cp.n_rows = g.n_rows;
+    cp.tiles_per_row = tiles_per_row;
+    cp.n_tiles = n_tiles;
+    cp.t_core_begin = int32_t(b);
+    cp.t_core_end = int32_t(e);
+    cp.t_origin = origin;
+    cp.tf_time_bins = g.tf_time_bins;
+    cp.theta = g.peak_min_q16;
+    cp.epoch = c->epoch;
+    cp.tile_bytes_max = c->tile_bytes_max;
+    cp.bm_words = c->bm_words;
+    const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->cluster_grid)));
+    k_cluster<<<grid, kThreads, c->smem_bytes, st>>>(cp);
+    c->launches++;
+  }
+  CK(c, cudaGetLastError());
+  CK(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));
+  c->last_stream = st;
+  c->run_pending = true;
+  c->last_n = n;
+  c->last_cap = cap;
+  return TPCCLUS_OK;
+}
+
+int tpcclus_result(tpcclus_ctx* c, tpcclus_run_stats* stats) {
+  if (!c || !stats) return TPCCLUS_ERR_INVALID;
+  std::memset(stats, 0, sizeof(*stats));
+  if (!c->run_pending) { stats->status = TPCCLUS_ERR_INVALID; return TPCCLUS_ERR_INVALID; }
+  cudaSetDevice(c->device);
+  cudaError_t e = cudaStreamSynchronize(c->last_stream);
+  c->run_pending = false;
+  stats->n_digits_in = c->last_n;
+  if (e != cudaSuccess) {
+    stats->status = TPCCLUS_ERR_CUDA;
+    stats->cuda_error = int(e);
+    return TPCCLUS_ERR_CUDA;
+  }
+  stats->n_digits_dropped = c->h_status->n_dropped;
+  stats->n_clusters = c->h_status->n_clusters;
+  int rc = TPCCLUS_OK;
+  if ((c->g.options & TPCCLUS_OPT_STRICT_DIGITS) && stats->n_digits_dropped) rc = TPCCLUS_ERR_DIGIT;
+  else if (stats->n_clusters > c->last_cap) rc = TPCCLUS_ERR_CAPACITY;
+  stats->status = rc;
+  return rc;
+}
+
+int tpcclus_run_tf_host(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf, tpcclus_cluster* h_out,
+                        uint64_t cap, tpcclus_run_stats* stats) {
+  if (!c || !fr || !stats || nf == 0 || (cap && !h_out)) return TPCCLUS_ERR_INVALID;
+  if (!(c->g.options & TPCCLUS_OPT_HOST_STAGING)) return TPCCLUS_ERR_INVALID;
+  for (uint32_t f = 0; f < nf; ++f)
+    if (fr[f].n > c->g.max_digits || (fr[f].n && !fr[f].h_digits) || !fr[f].h_sector_offsets) return TPCCLUS_ERR_INVALID;
+  CK(c, cudaSetDevice(c->device));
+  int first_err = TPCCLUS_OK;
+  uint64_t written = 0;
+  // prologue: H2D of fragment 0
+  CK(c, cudaMemcpyAsync(c->d_stage_digits[0], fr[0].h_digits, fr[0].n * sizeof(tpcclus_digit), cudaMemcpyHostToDevice, c->s_h2d));
+  CK(c, cudaEventRecord(c->ev_h2d[0], c->s_h2d));
+  for (uint32_t f = 0; f < nf; ++f) {
+    const int slot = int(f & 1u);
+    // kernels of fragment f: need its digits, and the slot's output buffer drained (D2H of f-2)
+    CK(c, cudaStreamWaitEvent(c->s_run, c->ev_h2d[slot], 0));
+    if (f >= 2) CK(c, cudaStreamWaitEvent(c->s_run, c->ev_d2h[slot], 0));
+    int rc = tpcclus_run(c, c->d_stage_digits[slot], fr[f].n, fr[f].h_sector_offsets, fr[f].t_core_begin,
+                         fr[f].t_core_end, c->d_stage_out[slot], c->g.max_clusters, c->s_run);
+    if (rc != TPCCLUS_OK) {
+      stats[f].status = rc;
+      return rc;
+    }
+    CK(c, cudaEventRecord(c->ev_run[slot], c->s_run));
+    // overlap: H2D of fragment f+1 into the other slot (free once the kernels of f-1 are done)
+    if (f + 1 < nf) {
+      const int nslot = slot ^ 1;
+      if (f >= 1) CK(c, cudaStreamWaitEvent(c->s_h2d, c->ev_run[nslot], 0));
+      CK(c, cudaMemcpyAsync(c->d_stage_digits[nslot], fr[f + 1].h_digits, fr[f + 1].n * sizeof(tpcclus_digit),
+                            cudaMemcpyHostToDevice, c->s_h2d));
+      CK(c, cudaEventRecord(c->ev_h2d[nslot], c->s_h2d));
+    }
+    // the record count decides the D2H size and where the next fragment's list starts (D10)
+    rc = tpcclus_result(c, &stats[f]);
+    if (rc == TPCCLUS_ERR_CUDA) return rc;
+    uint64_t ncopy = std::min<uint64_t>(stats[f].n_clusters, c->g.max_clusters);
+    if (written + ncopy > cap) { ncopy = cap - written; rc = TPCCLUS_ERR_CAPACITY; stats[f].status = rc; }
+    if (rc != TPCCLUS_OK && first_err == TPCCLUS_OK) first_err = rc;
+    if (ncopy) {
+      CK(c, cudaStreamWaitEvent(c->s_d2h, c->ev_run[slot], 0));
+      CK(c, cudaMemcpyAsync(h_out + written, c->d_stage_out[slot], ncopy * sizeof(tpcclus_cluster), cudaMemcpyDeviceToHost, c->s_d2h));
+    }
+    CK(c, cudaEventRecord(c->ev_d2h[slot], c->s_d2h));
+    written += ncopy;
+  }
+  CK(c, cudaStreamSynchronize(c->s_d2h));
+  CK(c, cudaStreamSynchronize(c->s_h2d));
+  return first_err;
+}
+
+int tpcclus_run_host(tpcclus_ctx* c, const tpcclus_digit* h_digits, uint64_t n, const uint64_t* h_off, uint32_t b,
+                     uint32_t e, tpcclus_cluster* h_out, uint64_t cap, tpcclus_run_stats* stats) {
+  tpcclus_fragment f;
+  f.h_digits = h_digits;
+  f.n = n;
+  f.h_sector_offsets = h_off;
+  f.t_core_begin = b;
+  f.t_core_end = e;
+  return tpcclus_run_tf_host(c, &f, 1, h_out, cap, stats);
+}
+
+uint64_t tpcclus_launch_count(const tpcclus_ctx* c) { return c ? c->launches : 0; }
+uint64_t tpcclus_device_bytes(const tpcclus_ctx* c) { return c ? c->dev_bytes : 0; }
+
+}  // extern "C"

@@ -1,0 +1,245 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI binding) against the oracle, element by
+element on the same seeded inputs, under the comparison rule D12 of SURVEY.md §8(c):
+integer fields, count and order bit-exact; qtot relative 1e-6; offsets and sigmas absolute 1e-4
+(BASELINE.json:north_star)."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from gpu_util import GpuClusterizer, gpu_clusters, oracle_clusters, to_device_digits
+from util import assert_clusters_match, count_bit_mismatches, digits_from_cells, permute_within_sectors
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def both(digits, offs, npads, **kw):
+    got, st = gpu_clusters(digits, offs, npads, **kw)
+    ref, ost = oracle_clusters(digits, offs, npads, **kw)
+    assert st["n_clusters"] == ost["n_clusters"]
+    assert st["n_digits_dropped"] == ost["n_digits_dropped"]
+    return got, ref, st
+
+
+PINS = json.load(open(os.path.join(HERE, "golden", "oracle_pins.json")))["pins"]
+
+
+@pytest.mark.parametrize("pin", PINS, ids=[p["name"] for p in PINS])
+def test_pins_on_gpu(pin):
+    """The hand-built maps P1..P9 through the CUDA path: same records as the oracle, bit for bit."""
+    d, offs = digits_from_cells([(0, 0, p, t, q) for p, t, q in pin["cells"]])
+    got, ref, _ = both(d, offs, [pin["npads"]], n_sectors=1, tf_time_bins=pin["tf_time_bins"],
+                       peak_min_q16=int(round(pin["theta_adc"] * 16)))
+    assert len(got) == len(pin["expect"])
+    assert_clusters_match(got, ref, pin["name"])
+    assert got.tobytes() == ref.tobytes()
+
+
+@pytest.mark.parametrize("theta", [1, 32, 64])
+def test_random_8x8_maps(theta):
+    """60000 random 8x8 maps with forced ties (the B2 family), packed as a 235 x 256 (sector,row)
+    grid of one run: tiny geometry, pad edges and time edges everywhere."""
+    rng = np.random.default_rng(2000 + theta)
+    n_maps, side = 60000, 8
+    alphabet = np.array([16, 32, 48, 64, 80, 96, 200, 16368], dtype=np.int64)
+    n_sectors = (n_maps + 255) // 256
+    q = rng.choice(alphabet, size=(n_maps, side, side))
+    fill = rng.choice([0.15, 0.3, 0.5, 0.8], size=n_maps)
+    keep = rng.random((n_maps, side, side)) < fill[:, None, None]
+    m, t, p = np.nonzero(keep)
+    d = np.zeros(len(m), dtype=oracle.DIGIT_DTYPE)
+    d["row"], d["pad"], d["time"] = m % 256, p, t
+    d["charge"] = q[m, t, p] / 16.0
+    offs = np.searchsorted(m // 256, np.arange(n_sectors + 1)).astype(np.uint64)
+    got, ref, _ = both(d, offs, [side] * 256, n_sectors=n_sectors, tf_time_bins=side, peak_min_q16=theta)
+    assert len(ref) > n_maps
+    assert_clusters_match(got, ref, "8x8")
+    assert count_bit_mismatches(got, ref) == 0
+
+
+def run_config(name, theta=64, **over):
+    cfg = gen.config(name, **over)
+    parts_g, parts_o = [], []
+    with GpuClusterizer(cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins,
+                        max_core_bins=cfg.core_bins, halo_bins=cfg.halo_bins, peak_min_q16=theta,
+                        max_digits=1 << 28) as g:
+        for f, (b, e) in enumerate(cfg.fragments()):
+            d, offs, info = gen.generate_fragment(cfg, f, device="cuda")
+            got, st = g.run(d, offs, b, e)
+            ref, ost = oracle_clusters(d, offs, cfg.npads_array(), n_sectors=cfg.n_sectors,
+                                       tf_time_bins=cfg.tf_time_bins, t_core_begin=b, t_core_end=e,
+                                       halo_bins=cfg.halo_bins, peak_min_q16=theta)
+            assert ost["n_duplicates"] == 0
+            assert st["n_clusters"] == ost["n_clusters"] and st["n_digits_dropped"] == ost["n_digits_dropped"] == 0
+            assert_clusters_match(got, ref, f"{cfg.name} fragment {f}")
+            parts_g.append(got)
+            parts_o.append(ref)
+    return cfg, np.concatenate(parts_g), np.concatenate(parts_o)
+
+
+@pytest.mark.parametrize("theta", [64, 32])
+def test_c0_tiny(theta):
+    """BASELINE.json:configs[0], full size, theta = 4 ADC and theta = ZS threshold (D11)."""
+    cfg, got, ref = run_config(0, theta)
+    assert len(ref) > 3000
+    assert count_bit_mismatches(got, ref) == 0
+
+
+def test_c1_pp_sector():
+    """BASELINE.json:configs[1], full size (1 sector x 4096 bins, ~2.2e6 digits)."""
+    cfg, got, ref = run_config(1)
+    assert len(ref) > 30000
+    assert count_bit_mismatches(got, ref) == 0
+
+
+@pytest.mark.parametrize("name,theta", [("c2mini", 64), ("c4mini", 64), ("c4mini", 32)])
+def test_pbpb_and_stress_minis(name, theta):
+    """The C2 and C4 generators on 2 sectors (several tiles per row, ragged last tile)."""
+    cfg, got, ref = run_config(name, theta)
+    assert len(ref) > 1e5
+    assert count_bit_mismatches(got, ref) == 0
+    if name == "c4mini":
+        assert (ref["flags"] & 8).any() and (ref["flags"] & 4).any() and (ref["flags"] & 1).any()
+
+
+def test_c3mini_fragmented_tf():
+    """configs[3] in small: 3 fragments (512,512,476 bins) with an 8-bin halo; the concatenated
+    fragment lists equal the monolithic oracle run (D9/D10, invariant I7)."""
+    cfg, got, ref = run_config("c3mini")
+    mono = gen.config("c3mini", core_bins=cfg.tf_time_bins, halo_bins=0)
+    d, offs, _ = gen.generate_fragment(mono, 0, device="cuda")
+    full, _ = oracle_clusters(d, offs, mono.npads_array(), n_sectors=mono.n_sectors, tf_time_bins=mono.tf_time_bins)
+    k = np.lexsort((got["pad"], got["time"], got["row"], got["sector"]))
+    assert_clusters_match(got[k], full, "fragmented vs monolithic")
+
+
+def test_determinism_and_permutation():
+    """I3 + the determinism guarantee: two runs and a permuted-input run are byte-identical."""
+    cfg = gen.config("c4mini", tf_time_bins=300, core_bins=300)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    a, _ = gpu_clusters(dn, offs, cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    b, _ = gpu_clusters(dn, offs, cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    p = permute_within_sectors(dn, offs, np.random.default_rng(5))
+    c, _ = gpu_clusters(p, offs, cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    assert len(a) > 1e4 and a.tobytes() == b.tobytes() == c.tobytes()
+    key = (a["sector"].astype(np.int64) << 48) | (a["row"].astype(np.int64) << 40) | \
+          (a["time"].astype(np.int64) << 8) | a["pad"]
+    assert np.all(np.diff(key) > 0)
+
+
+def test_odd_core_sizes_and_halo():
+    """Any core size with halo >= 5 (ragged tiles, core of 1 bin, core not a multiple of the tile)."""
+    cfg = gen.config(0, n_rows=5, tf_time_bins=700, core_bins=700, clusters_per_row=120)
+    d, offs, _ = gen.generate_fragment(cfg, 0)
+    dn = gen.as_numpy_digits(d)
+    dd = to_device_digits(dn)
+    npads = cfg.npads_array()
+    for core, halo in [(1, 5), (129, 5), (257, 8), (700, 0)]:
+        with GpuClusterizer(npads, n_sectors=1, tf_time_bins=700, max_core_bins=core, halo_bins=halo,
+                            max_digits=len(dn)) as g:
+            for b in ([0, 313, 699] if core == 1 else range(0, 700, core)):
+                e = min(700, b + core)
+                got, st = g.run(dd, offs, b, e)
+                ref, ost = oracle.run(dn, offs, npads, n_sectors=1, tf_time_bins=700, t_core_begin=b,
+                                      t_core_end=e, halo_bins=halo)
+                assert st["n_digits_dropped"] == ost["n_digits_dropped"]
+                assert_clusters_match(got, ref, f"core {core} halo {halo} b {b}")
+                assert got.tobytes() == ref.tobytes()
+
+
+def test_empty_and_degenerate_inputs():
+    import paper_2412_13755_b200 as T
+
+    npads = [10, 1, 248]
+    empty = np.zeros(0, dtype=oracle.DIGIT_DTYPE)
+    got, st = gpu_clusters(empty, np.zeros(3, dtype=np.uint64), npads, n_sectors=2, tf_time_bins=40)
+    assert len(got) == 0 and st["n_clusters"] == 0
+    # single digit in the widest row's last pad, last time bin; a 1-pad row; dropped digits
+    cells = [(1, 2, 247, 39, 9.0), (0, 1, 0, 0, 5.0), (0, 1, 0, 1, 5.0), (0, 0, 10, 3, 50.0),
+             (0, 3, 1, 1, 50.0), (1, 0, 2, 40, 50.0), (1, 0, 3, 3, float("nan")), (1, 0, 4, 3, 0.01)]
+    d, offs = digits_from_cells(cells, n_sectors=2)
+    got, ref, st = both(d, offs, npads, n_sectors=2, tf_time_bins=40)
+    assert st["n_digits_dropped"] == 5 and len(ref) == 2
+    assert got.tobytes() == ref.tobytes()
+    # strict mode turns dropped digits into an error
+    with GpuClusterizer(npads, n_sectors=2, tf_time_bins=40, max_digits=16,
+                        options=T.TPCCLUS_OPT_STRICT_DIGITS) as g:
+        _, st = g.run(to_device_digits(d), offs, 0, 40, capacity=8, check=False)
+        assert st["status"] == T.TPCCLUS_ERR_DIGIT
+
+
+def test_capacity_overflow_is_ordered_prefix():
+    """ERR_CAPACITY: the first out_capacity records are valid and ordered, n_clusters = required."""
+    import paper_2412_13755_b200 as T
+
+    cfg = gen.config(0, n_rows=6, tf_time_bins=256, core_bins=256, clusters_per_row=60)
+    d, offs, _ = gen.generate_fragment(cfg, 0)
+    dn = gen.as_numpy_digits(d)
+    ref, _ = oracle.run(dn, offs, cfg.npads_array(), n_sectors=1, tf_time_bins=256)
+    with GpuClusterizer(cfg.npads_array(), n_sectors=1, tf_time_bins=256, max_digits=len(dn)) as g:
+        got, st = g.run(to_device_digits(dn), offs, 0, 256, capacity=100, check=False)
+    assert st["status"] == T.TPCCLUS_ERR_CAPACITY and st["n_clusters"] == len(ref) > 100
+    assert got.tobytes() == ref[:100].tobytes()
+
+
+def test_invalid_arguments():
+    import torch
+    import paper_2412_13755_b200 as T
+
+    with pytest.raises(T.TpcclusError) as ei:
+        T.tpcclus_create([10, 300], n_sectors=1, tf_time_bins=100, max_digits=10)
+    assert ei.value.code == T.TPCCLUS_ERR_GEOMETRY
+    with pytest.raises(T.TpcclusError) as ei:
+        T.tpcclus_create([10], n_sectors=1, tf_time_bins=100, halo_bins=3, max_digits=10)
+    assert ei.value.code == T.TPCCLUS_ERR_GEOMETRY
+    ctx = T.tpcclus_create([10], n_sectors=1, tf_time_bins=100, max_core_bins=50, max_digits=10)
+    try:
+        buf = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        offs = np.array([0, 2], dtype=np.uint64)
+        for args in [(buf.data_ptr(), 2, offs, 0, 60, 0, 0),             # core larger than max_core_bins
+                     (buf.data_ptr(), 2, offs, 90, 120, 0, 0),           # core outside the TF
+                     (buf.data_ptr(), 2, np.array([0, 1], dtype=np.uint64), 0, 50, 0, 0),  # off[n] != n
+                     (buf.data_ptr() + 4, 2, offs, 0, 50, 0, 0),         # misaligned digits
+                     (buf.data_ptr(), 11, np.array([0, 11], dtype=np.uint64), 0, 50, 0, 0)]:  # n > max_digits
+            with pytest.raises(T.TpcclusError) as ei:
+                T.tpcclus_run(ctx, *args)
+            assert ei.value.code == T.TPCCLUS_ERR_INVALID
+    finally:
+        T.tpcclus_destroy(ctx)
+
+
+def test_host_api_single_and_tf():
+    """tpcclus_run_host / tpcclus_run_tf_host: host buffers in, host records out, fragments
+    concatenated in order (D10)."""
+    import paper_2412_13755_b200 as T
+
+    cfg = gen.config("c3mini", n_sectors=2)
+    frs, keep, refs = [], [], []
+    for f, (b, e) in enumerate(cfg.fragments()):
+        d, offs, _ = gen.generate_fragment(cfg, f)
+        dn = gen.as_numpy_digits(d)
+        keep.append(dn)
+        frs.append((dn.ctypes.data, len(dn), offs, b, e))
+        ref, _ = oracle.run(dn, offs, cfg.npads_array(), n_sectors=2, tf_time_bins=cfg.tf_time_bins,
+                            t_core_begin=b, t_core_end=e, halo_bins=8)
+        refs.append(ref)
+    total = sum(len(r) for r in refs)
+    ctx = T.tpcclus_create(cfg.npads_array(), n_sectors=2, tf_time_bins=cfg.tf_time_bins, max_core_bins=512,
+                           halo_bins=8, options=T.TPCCLUS_OPT_HOST_STAGING,
+                           max_digits=max(len(k) for k in keep), max_clusters=max(len(r) for r in refs) + 10)
+    try:
+        out = np.zeros(total, dtype=T.CLUSTER_DTYPE)
+        stats = T.tpcclus_run_tf_host(ctx, frs, out.ctypes.data, total)
+        assert [s["n_clusters"] for s in stats] == [len(r) for r in refs]
+        assert out.tobytes() == np.concatenate(refs).tobytes()
+        one = np.zeros(len(refs[1]), dtype=T.CLUSTER_DTYPE)
+        st = T.tpcclus_run_host(ctx, keep[1], frs[1][2], frs[1][3], frs[1][4], one)
+        assert st["n_clusters"] == len(refs[1]) and one.tobytes() == refs[1].tobytes()
+        assert T.tpcclus_launch_count(ctx) == 3 * 4 and T.tpcclus_device_bytes(ctx) > 0
+    finally:
+        T.tpcclus_destroy(ctx)
