@@ -37,7 +37,7 @@ extern "C" {
 #define TPCCLUS_OK             0
 #define TPCCLUS_ERR_INVALID   -1  /* null / misaligned pointer, core range larger than max_core_bins,
                                      core outside the TF, offsets not monotone, n > max_digits       */
-#define TPCCLUS_ERR_GEOMETRY  -2  /* npads out of 1..248, zero sizes, halo_bins in 1..4, tf > 65536   */
+#define TPCCLUS_ERR_GEOMETRY  -2  /* npads out of 1..246, zero sizes, halo_bins in 1..4, tf > 65536   */
 #define TPCCLUS_ERR_CAPACITY  -3  /* more clusters than out_capacity: the first out_capacity records
                                      are valid and ordered, stats.n_clusters is the number required
                                      (hit count fluctuates -> "safety margin")         */
@@ -59,7 +59,7 @@ extern "C" {
                                              (2 x max_digits digits + 2 x max_clusters records) */
 
 #define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
-#define TPCCLUS_MAX_NPADS  248u
+#define TPCCLUS_MAX_NPADS  246u  /* 8 + npads + 2 columns must fit a 256-wide TMA box */
 #define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
 
 /* One zero-suppressed digit, 8 bytes (BASELINE.json:configs[0]: "uint8 row, uint8 pad,

@@ -9,6 +9,7 @@
 #include "tpcclus_kernels.cuh"
 
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -65,6 +66,19 @@ inline uint32_t roundup(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
 int cuda_fail(tpcclus_ctx* c, cudaError_t e) {
   if (c) { c->sticky = TPCCLUS_ERR_CUDA; c->sticky_cuda = int(e); }
   return TPCCLUS_ERR_CUDA;
+}
+
+// TPCCLUS_DEBUG=1 in the environment: synchronise after every launch and name the kernel that
+// failed on stderr (debugging aid; never set in tests or the bench).
+bool debug_sync() {
+  static const bool on = [] { const char* v = std::getenv("TPCCLUS_DEBUG"); return v && v[0] == '1'; }();
+  return on;
+}
+void debug_check(cudaStream_t st, const char* what) {
+  if (!debug_sync()) return;
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  std::fprintf(stderr, "[tpcclus] %s: %s\n", what, cudaGetErrorString(e));
 }
 
 #define CK(ctx, call)                                  \
@@ -153,7 +167,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     RowInfo& ri = c->rows[r];
     ri.npads = c->npads[r];
     ri.pitch = uint16_t(roundup(ri.npads, 8));
-    ri.boxw = uint16_t(roundup(ri.npads + 2 * kPadHalo, 8));
+    ri.boxw = uint16_t(roundup(kPadHalo + ri.npads + kPadTail, 8));
     ri.nwords = uint16_t((ri.npads + 1) / 2);
     if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
     ri.map_off = uint32_t(off);
@@ -167,8 +181,8 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * ((g->max_core_bins + kTileT - 1) / kTileT);
   if (tiles > 0x7FFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
-  c->smem_bytes = kStages * c->tile_bytes_max + kBoxH * c->bm_words * 4 + (kTileT + 1) * 4 + kListCap * 4 +
-                  256 * sizeof(RowInfo) + kStages * 8 + kStages * 4 + 16 * 4 + 128;
+  c->smem_bytes = kStages * c->tile_bytes_max + 16 * 8 + 16 * 4 + 16 * 4 + kListCap * 4 + 256 * sizeof(RowInfo) +
+                  (kTileT + 4) * 4 + kBoxH * c->bm_words * 4 + 128;
 
   int rc;
   const uint64_t map_bytes = uint64_t(g->n_sectors) * c->sec_elems * 2;
@@ -269,6 +283,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     dim3 grid(g.n_sectors * g.n_rows, chunks);
     k_clear<<<grid, 256, 0, st>>>(c->d_map, c->d_rows, g.n_rows, c->sec_elems, rows_used, c->d_status);
     c->launches++;
+    debug_check(st, "k_clear");
   }
   // S1: scatter
   if (n) {
@@ -285,6 +300,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     const uint32_t blocks = uint32_t(std::min<uint64_t>((pairs + 255) / 256, uint64_t(c->n_sm) * 16));
     k_scatter<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), sp, c->d_rows, c->d_map, c->d_status);
     c->launches++;
+    debug_check(st, "k_scatter");
   }
   // S2..S7: fused tile kernel
   {
@@ -310,6 +326,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->cluster_grid)));
     k_cluster<<<grid, kThreads, c->smem_bytes, st>>>(cp);
     c->launches++;
+    debug_check(st, "k_cluster");
   }
   CK(c, cudaGetLastError());
   CK(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));

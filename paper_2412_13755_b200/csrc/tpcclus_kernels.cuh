@@ -24,7 +24,9 @@ constexpr int      kThreads      = 256;   // CTA size of k_cluster
 constexpr int      kTileT        = 128;   // core time bins per tile
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // tile rows staged in smem
-constexpr int      kPadHalo      = 2;     // box starts at pad -2 (5x5 window); flags need no charge halo
+constexpr int      kPadHalo      = 8;     // box starts at pad -8: the innermost TMA coordinate must be a multiple
+                                          // of 16 bytes (measured: -2 raises 'illegal instruction'); 2 would do for 5x5
+constexpr int      kPadTail      = 2;     // cells kept right of the last pad (5x5 window)
 constexpr int      kStages       = 2;     // TMA double buffering
 constexpr int      kListCap      = 1024;  // peaks processed per pass inside one tile
 constexpr uint32_t kQClamp       = 16368; // D1
@@ -34,7 +36,7 @@ struct RowInfo {              // one per pad row (device table)
   uint32_t map_off;           // element offset of this row's [H][pitch] block inside one sector's map
   uint16_t npads;
   uint16_t pitch;             // elements, multiple of 8 (TMA: global stride multiple of 16 bytes)
-  uint16_t boxw;              // TMA box width in elements = roundup8(npads + 2*kPadHalo)
+  uint16_t boxw;              // TMA box width in elements = roundup8(kPadHalo + npads + kPadTail)
   uint16_t nwords;            // active 2-cell word columns = ceil(npads/2)
 };
 
@@ -111,6 +113,12 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* t
           "r"(smem_u32(smem_dst)),
       "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(x), "r"(y)
       : "memory");
+}
+// The descriptors live in global memory (written once by the host in tpcclus_create); make them
+// visible to the tensormap proxy of this SM before the first TMA that uses them.
+__device__ __forceinline__ void tensormap_fence_acquire(const CUtensorMap* tmap) {
+  asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(reinterpret_cast<uint64_t>(tmap))
+               : "memory");
 }
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
   unsigned long long v;
@@ -282,7 +290,7 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
                                               uint32_t tf_time_bins, ClusterRec& rec) {
   // 5x5 charges around the peak: box column of pad p is p + kPadHalo
   uint32_t q[5][5];
-  const uint16_t* c0 = tile + (j - 2) * boxw + pad;          // column (pad + 2) - 2
+  const uint16_t* c0 = tile + (j - 2) * boxw + (pad + kPadHalo - 2);
 #pragma unroll
   for (int dt = 0; dt < 5; ++dt)
 #pragma unroll
@@ -365,17 +373,17 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
 __global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__ ClusterParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
-  uint8_t* sp = smem_raw;
+  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // TMA destination: 128-byte aligned
   uint16_t* tile_buf[kStages];
 #pragma unroll
   for (int s = 0; s < kStages; ++s) { tile_buf[s] = reinterpret_cast<uint16_t*>(sp); sp += P.tile_bytes_max; }
-  uint32_t* bm = reinterpret_cast<uint32_t*>(sp);           sp += kBoxH * P.bm_words * 4;
-  uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 1) * 4;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += 16 * 8;        // kStages used, keeps 128-byte alignment
+  uint32_t* s_tile = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // tile id per stage
+  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // [0] exclusive prefix, [1..8] warp totals
   uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
   RowInfo* srow = reinterpret_cast<RowInfo*>(sp);           sp += 256 * sizeof(RowInfo);
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += kStages * 8;
-  uint32_t* s_tile = reinterpret_cast<uint32_t*>(sp);       sp += kStages * 4;   // tile id per stage
-  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       // [0] exclusive prefix, [1] warp-scan scratch[8]
+  uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
+  uint32_t* bm = reinterpret_cast<uint32_t*>(sp);
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   for (uint32_t i = tid; i < P.n_rows; i += kThreads) srow[i] = P.rows[i];
@@ -394,6 +402,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__
       const uint32_t row = sr % P.n_rows;
       const RowInfo ri = srow[row];
       const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;
+      tensormap_fence_acquire(P.tmaps + sr);
       mbar_arrive_expect_tx(&mbar[s], uint32_t(kBoxH) * ri.boxw * 2u);
       tma_load_2d(tile_buf[s], P.tmaps + sr, -kPadHalo, (t0 - P.t_origin) - kReach, &mbar[s]);
     }
@@ -429,18 +438,18 @@ __global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__
     // horizontal maxima of the previous / current / next row in registers.
     {
       const uint32_t wpr = ri.boxw >> 1;                 // 32-bit words per tile row
-      const uint32_t nw = ri.nwords;                     // active word columns (word 1 .. nw)
+      const uint32_t nw = ri.nwords;                     // active word columns (pads 0 .. npads-1)
       const uint32_t nstrips = kThreads / nw;
       const uint32_t strip = tid / nw, wc = tid - strip * nw;
       const uint32_t R = ncore + 2 * (kReach - 1);       // rows 1..R get flags
       const uint32_t rps = (R + nstrips - 1) / nstrips;
       const uint32_t jb = 1 + strip * rps, je = min(jb + rps, R + 1);
       if (strip < nstrips && jb < je) {
-        const uint32_t* t32 = reinterpret_cast<const uint32_t*>(tile) + (wc + 1);
+        const uint32_t* t32 = reinterpret_cast<const uint32_t*>(tile) + (wc + kPadHalo / 2);
         const uint32_t theta2 = P.theta | (P.theta << 16);
         auto load3 = [&](uint32_t j, uint32_t& X, uint32_t& L, uint32_t& Rr) {
           const uint32_t* p = t32 + j * wpr;
-          const uint32_t xl = p[-1], xr = p[1];          // word 0 and word wpr-1 are pure halo
+          const uint32_t xl = p[-1], xr = p[1];          // halo words left and right are zero
           X = p[0];
           L = __byte_perm(xl, X, 0x5432);                // (pad-1, pad) for the low half, ...
           Rr = __byte_perm(X, xr, 0x5432);               // (pad+1, pad+2)
@@ -461,7 +470,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__
           const uint32_t bound = __vimax3_u16x2(be, bl, theta2);
           const uint32_t pk = ((X | 0x80008000u) - bound) & 0x80008000u;   // bit15 of a half: Q >= bound
           if (pk) {
-            const uint32_t bit0 = 2u * (wc + 1) - kPadHalo + 4u;           // bitmap bit = pad + 4
+            const uint32_t bit0 = 2u * wc + 4u;                            // bitmap bit = pad + 4
             if (pk & 0x00008000u) atomicOr(&bm[j * bmw + (bit0 >> 5)], 1u << (bit0 & 31u));
             if (pk & 0x80000000u) atomicOr(&bm[j * bmw + ((bit0 + 1) >> 5)], 1u << ((bit0 + 1) & 31u));
           }

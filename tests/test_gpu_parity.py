@@ -155,12 +155,12 @@ def test_odd_core_sizes_and_halo():
 def test_empty_and_degenerate_inputs():
     import paper_2412_13755_b200 as T
 
-    npads = [10, 1, 248]
+    npads = [10, 1, 246]
     empty = np.zeros(0, dtype=oracle.DIGIT_DTYPE)
     got, st = gpu_clusters(empty, np.zeros(3, dtype=np.uint64), npads, n_sectors=2, tf_time_bins=40)
     assert len(got) == 0 and st["n_clusters"] == 0
     # single digit in the widest row's last pad, last time bin; a 1-pad row; dropped digits
-    cells = [(1, 2, 247, 39, 9.0), (0, 1, 0, 0, 5.0), (0, 1, 0, 1, 5.0), (0, 0, 10, 3, 50.0),
+    cells = [(1, 2, 245, 39, 9.0), (0, 1, 0, 0, 5.0), (0, 1, 0, 1, 5.0), (0, 0, 10, 3, 50.0),
              (0, 3, 1, 1, 50.0), (1, 0, 2, 40, 50.0), (1, 0, 3, 3, float("nan")), (1, 0, 4, 3, 0.01)]
     d, offs = digits_from_cells(cells, n_sectors=2)
     got, ref, st = both(d, offs, npads, n_sectors=2, tf_time_bins=40)
