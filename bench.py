@@ -1,0 +1,434 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the TPC cluster finder on synthetic Pb-Pb time frames.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+A "step" is one pass of the whole hot path (S0..S7 of SURVEY.md §8(a)) over one time frame:
+for BASELINE.json:configs[3] that is 14 fragments (13 x 4096 + 3776 bins, 8-bin halo) of
+36 sectors, ~4.4e9 digits, resident in HBM when the timed region starts.  Prints ONE JSON
+line (rank 0).  Multi-GPU (torchrun): the path does not shard (BASELINE.json:north_star:
+"one GPU only, no sharding"), so N ranks run N independent replicas ("replicas only").
+
+--impl reference times the ORACLE (oracle/, plain single-threaded C++ per call, one sector per
+host thread) on a bounded sample of the same workload; it is a baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tpc_digits_per_sec"
+UNIT = "digits/s"
+THETA = 64          # peak_min_q16 = 4 ADC (D11 default)
+
+
+def log(*a):
+    print("[bench]", *a, file=sys.stderr, flush=True)
+
+
+# ----------------------------------------------------------------------------------------------
+# distributed plumbing (replicas only): barrier + max over ranks
+# ----------------------------------------------------------------------------------------------
+def dist_setup(backend=None):
+    """Returns (rank, world, local_rank).  Initialises torch.distributed when WORLD_SIZE > 1."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+
+        if not dist.is_initialized():
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            dist.init_process_group(backend or "nccl", rank=rank, world_size=world)
+    return rank, world, local
+
+
+def dist_barrier(world, device=None):
+    if world > 1:
+        import torch.distributed as dist
+
+        if device is not None and dist.get_backend() == "nccl":
+            dist.barrier(device_ids=[device])
+        else:
+            dist.barrier()
+
+
+def dist_max_sum(ms: float, units: float, world: int, device="cpu"):
+    """(max over ranks of the elapsed time, sum over ranks of the units processed)."""
+    if world == 1:
+        return ms, units
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ----------------------------------------------------------------------------------------------
+# clocks (profiling recipe: sample nvidia-smi DURING the timed region)
+# ----------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown," \
+        "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown," \
+        "clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm))
+        return out
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------------------
+# workload
+# ----------------------------------------------------------------------------------------------
+def make_tf(cfg, device, frags=None):
+    import gen
+
+    out = []
+    t0 = time.time()
+    for f, (b, e) in enumerate(cfg.fragments()):
+        if frags is not None and f not in frags:
+            continue
+        d, offs, info = gen.generate_fragment(cfg, f, device=device,
+                                              row_chunk=64 if str(device).startswith("cuda") else 16)
+        out.append(dict(f=f, b=b, e=e, digits=d, offs=offs, n=int(d.shape[0]), occ=info["occupancy"]))
+    log(f"generated {cfg.name}: {len(out)} fragments, {sum(x['n'] for x in out):,} digits, "
+        f"mean occupancy {np.mean([x['occ'] for x in out]):.4f}, {time.time() - t0:.1f} s on {device}")
+    return out
+
+
+def oracle_sample(cfg, frag, sectors, threads):
+    """Run the oracle on `sectors` of one fragment, one sector per call, `threads` calls in
+    parallel.  Returns (seconds, digits processed, {sector: records})."""
+    import oracle
+
+    dn = frag["digits_np"]
+    offs = frag["offs"]
+    npads = cfg.npads_array()
+
+    def one(s):
+        a, b_ = int(offs[s]), int(offs[s + 1])
+        rec, st = oracle.run(dn[a:b_], np.array([0, b_ - a], dtype=np.uint64), npads, n_sectors=1,
+                             tf_time_bins=cfg.tf_time_bins, t_core_begin=frag["b"], t_core_end=frag["e"],
+                             halo_bins=cfg.halo_bins, peak_min_q16=THETA)
+        return s, rec
+
+    oracle.build()
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        res = dict(ex.map(one, sectors))
+    dt = time.perf_counter() - t0
+    nd = int(sum(int(offs[s + 1]) - int(offs[s]) for s in sectors))
+    return dt, nd, res
+
+
+# ----------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle as it stands, on the box's host cores, on a bounded sample per step."""
+    rank, world, local = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), 0
+    if rank != 0:
+        return
+    import torch
+    import gen
+
+    cfg = gen.config(args.config)
+    cores = os.cpu_count() or 1
+    n_s = min(cfg.n_sectors, cores)
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    import gen as _g
+    d, offs, info = _g.generate_fragment(cfg, 0, device=dev, sectors=range(n_s),
+                                         row_chunk=64 if dev != "cpu" else 16)
+    b, e = cfg.fragments()[0]
+    frag = dict(b=b, e=e, offs=offs, digits_np=_g.as_numpy_digits(d))
+    times, nd, ncl = [], 0, 0
+    for i in range(args.warmup + args.steps):
+        dt, nd, res = oracle_sample(cfg, frag, list(range(n_s)), cores)
+        ncl = sum(len(r) for r in res.values())
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    val = nd / (ms * 1e-3)
+    sample = f"{n_s} of {cfg.n_sectors} sectors of fragment 0 ({nd:,} digits), one sector per thread"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64/f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "clusters_per_sec": ncl / (ms * 1e-3),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": min(cores, n_s), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }), flush=True)
+
+
+def workload_name(cfg):
+    fr = cfg.fragments()
+    return (f"{cfg.name}: {cfg.n_sectors} sectors x {cfg.n_rows} rows x {cfg.tf_time_bins} time bins, "
+            f"{len(fr)} fragment(s) of <= {cfg.core_bins} bins, halo {cfg.halo_bins}, seed {cfg.seed}, theta 4 ADC")
+
+
+def run_ours(args):
+    import torch
+    import gen
+    import paper_2412_13755_b200 as T
+
+    rank, world, local = dist_setup()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    cfg = gen.config(args.config)
+    npads = cfg.npads_array()
+    tf = make_tf(cfg, dev)
+    n_dig = sum(x["n"] for x in tf)
+    max_n = max(x["n"] for x in tf)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    ctx = T.tpcclus_create(npads, n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins,
+                           max_core_bins=cfg.core_bins, halo_bins=cfg.halo_bins, peak_min_q16=THETA,
+                           max_digits=max_n, cuda_device=local)
+    # count pass (capacity 0): cluster counts per fragment -> exact output sizing
+    for x in tf:
+        T.tpcclus_run(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["b"], x["e"], 0, 0, stream)
+    counts = []
+    for x in tf:
+        st = T.tpcclus_result(ctx, check=False)
+        assert st["status"] in (T.TPCCLUS_OK, T.TPCCLUS_ERR_CAPACITY) and st["n_digits_dropped"] == 0, st
+        counts.append(int(st["n_clusters"]))
+    n_cl = sum(counts)
+    starts = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    out = torch.zeros((max(n_cl, 1), 32), dtype=torch.uint8, device=dev)
+    log(f"{n_dig:,} digits -> {n_cl:,} clusters; context holds {T.tpcclus_device_bytes(ctx) / 1e9:.2f} GB")
+
+    def step():
+        for i, x in enumerate(tf):
+            T.tpcclus_run(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["b"], x["e"],
+                          out.data_ptr() + int(starts[i]) * 32, counts[i], stream)
+        for i in range(len(tf)):
+            st = T.tpcclus_result(ctx)
+            assert st["n_clusters"] == counts[i]
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    dist_barrier(world, local)
+    T.tpcclus_set_profiling(ctx, True)
+    launches0 = T.tpcclus_launch_count(ctx)
+    clocks = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize()
+    dist_barrier(world, local)
+    ms_total = ev0.elapsed_time(ev1)
+    clk = clocks.stop()
+    launches = T.tpcclus_launch_count(ctx) - launches0
+    prof, prof_runs = T.tpcclus_get_profile(ctx)
+    T.tpcclus_set_profiling(ctx, False)
+    ms_step_local = ms_total / args.steps
+    ms_step, units = dist_max_sum(ms_step_local, float(n_dig), world, dev)
+    value = units / (ms_step * 1e-3)
+
+    if rank != 0:
+        T.tpcclus_destroy(ctx)
+        return
+
+    # ---- roofline of the dominant kernel (algorithmic bytes per launch / mean launch time) ----
+    peak, peak_src = measured_peak_gbs()
+    cells_core = int(npads.astype(np.int64).sum()) * cfg.n_sectors * sum(x["e"] - x["b"] for x in tf)
+    rows_used = [min(cfg.core_bins + 2 * cfg.halo_bins,
+                     ((x["e"] - x["b"] + 127) // 128) * 128 + cfg.halo_bins + 5) for x in tf]
+    pitch_sum = int(((npads.astype(np.int64) + 7) // 8 * 8).sum())
+    cells_cleared = sum(pitch_sum * cfg.n_sectors * r for r in rows_used)
+    nfr = len(tf)
+    alg = {   # bytes per launch, DESIGN.md §6
+        "k_clear": 2.0 * cells_cleared / nfr,                     # store every cell of the used rows once
+        "k_scatter": (8.0 + 2.0) * n_dig / nfr,                   # read 8 B/digit, write 2 B/digit
+        "k_cluster": (2.0 * cells_core + 32.0 * n_cl) / nfr,      # read every core cell once, write every record
+    }
+    kern = {}
+    for k, ms_sum in prof.items():
+        ms_avg = ms_sum / max(prof_runs, 1)
+        kern[k] = dict(ms_per_launch=ms_avg, alg_bytes_per_launch=alg[k],
+                       achieved_gbs=alg[k] / (ms_avg * 1e-3) / 1e9 if ms_avg > 0 else None,
+                       share=ms_sum / max(sum(prof.values()), 1e-9))
+    dom = max(kern, key=lambda k: kern[k]["ms_per_launch"])
+    traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(dom) \
+        if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else None
+    roofline = dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
+                    frac=kern[dom]["achieved_gbs"] / peak, traffic=traffic, peak_source=peak_src,
+                    kernels=kern,
+                    whole_step=dict(
+                        b_min_bytes=8.0 * n_dig + 32.0 * n_cl,
+                        frac_b_min=(8.0 * n_dig + 32.0 * n_cl) / (ms_step_local * 1e-3) / 1e9 / peak,
+                        frac_b_min_nominal_8tbs=(8.0 * n_dig + 32.0 * n_cl) / (ms_step_local * 1e-3) / 1e9 / 8000.0,
+                        b_alg_bytes=sum(alg.values()) * nfr,
+                        frac_b_alg=sum(alg.values()) * nfr / (ms_step_local * 1e-3) / 1e9 / peak))
+
+    # ---- cpu baseline (oracle, bounded sample) + parity spot check at full size ----
+    cpu, parity = None, None
+    if world == 1 and not args.no_cpu:
+        cores = os.cpu_count() or 1
+        n_s = min(cfg.n_sectors, max(cores, 1) * 2)
+        f0 = tf[0]
+        a, b_ = 0, int(f0["offs"][n_s])
+        frag = dict(b=f0["b"], e=f0["e"], offs=f0["offs"],
+                    digits_np=gen.as_numpy_digits(f0["digits"][a:b_]))
+        dt, nd, res = oracle_sample(cfg, frag, list(range(n_s)), cores)
+        sample = f"{n_s} of {cfg.n_sectors} sectors of fragment 0 ({nd:,} digits), one sector per thread"
+        cpu = dict(value=nd / dt, unit=UNIT, cores=min(cores, n_s), kind="oracle", sample=sample, seconds=dt)
+        got = out[: counts[0]].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)
+        bad, nrec = 0, 0
+        for s, rec in res.items():
+            g = got[got["sector"] == s].copy()
+            g["sector"] = 0
+            nrec += len(rec)
+            bad += (len(g) != len(rec)) or (g.tobytes() != rec.tobytes())
+        parity = dict(fragment=0, sectors=n_s, records=nrec, sectors_not_bit_identical=int(bad))
+
+    # ---- end to end through the C-ABI with HOST buffers (H2D + kernels + D2H inside the timing) ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            e2e = run_e2e(args, cfg, tf, counts, T, local, world)
+        except Exception as ex:  # report, never fake
+            log("e2e failed:", repr(ex))
+            e2e = dict(value=None, unit=UNIT, error=repr(ex))
+
+    T.tpcclus_destroy(ctx)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u16 charges, int32/int64 moments, f64 finish", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "digits_per_step": n_dig, "clusters_per_step": n_cl,
+                   "l2": "inputs larger than L2 (digits %.1f GB per step, map %.1f GB per fragment)"
+                         % (n_dig * 8 / 1e9, 2.0 * cells_cleared / nfr / 1e9),
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "clusters_per_sec": n_cl * world / (ms_step * 1e-3),
+        "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roofline, "cpu_baseline": cpu, "parity_check": parity,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_e2e(args, cfg, tf, counts, T, local, world):
+    import torch
+
+    npads = cfg.npads_array()
+    n_dig, n_cl = sum(x["n"] for x in tf), sum(counts)
+    ctx = T.tpcclus_create(npads, n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins,
+                           max_core_bins=cfg.core_bins, halo_bins=cfg.halo_bins, peak_min_q16=THETA,
+                           options=T.TPCCLUS_OPT_HOST_STAGING, max_digits=max(x["n"] for x in tf),
+                           max_clusters=max(counts) + 1, cuda_device=local)
+    try:
+        t0 = time.time()
+        hosts = []
+        for x in tf:
+            h = torch.empty((x["n"], 8), dtype=torch.uint8, pin_memory=True)
+            h.copy_(x["digits"])
+            hosts.append(h)
+        h_out = torch.empty((max(n_cl, 1), 32), dtype=torch.uint8, pin_memory=True)
+        torch.cuda.synchronize()
+        log(f"e2e: pinned {n_dig * 8 / 1e9:.1f} GB of digits + {n_cl * 32 / 1e9:.1f} GB of records on the host in {time.time() - t0:.1f} s")
+        frs = [(h.data_ptr(), x["n"], x["offs"], x["b"], x["e"]) for h, x in zip(hosts, tf)]
+        n_e2e = max(1, min(args.steps, 3))
+        for _ in range(1):
+            st = T.tpcclus_run_tf_host(ctx, frs, h_out.data_ptr(), n_cl)
+        assert [s["n_clusters"] for s in st] == counts
+        dist_barrier(world, local)
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            T.tpcclus_run_tf_host(ctx, frs, h_out.data_ptr(), n_cl)   # returns after the last D2H
+        dt = (time.perf_counter() - t0) / n_e2e
+        dist_barrier(world, local)
+        ms, units = dist_max_sum(dt * 1e3, float(n_dig), world, f"cuda:{local}")
+        return dict(value=units / (ms * 1e-3), unit=UNIT, ms_per_step=ms, steps=n_e2e,
+                    h2d_bytes_per_step=int(n_dig * 8), d2h_bytes_per_step=int(n_cl * 32),
+                    api="tpcclus_run_tf_host, pinned host buffers; H2D, kernels and D2H overlapped across fragments")
+    finally:
+        T.tpcclus_destroy(ctx)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="3", help="BASELINE.json config index 0..4 (default 3: the full Pb-Pb TF)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    args.config = int(args.config) if args.config.isdigit() else args.config
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

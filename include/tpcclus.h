@@ -60,6 +60,7 @@ extern "C" {
 
 #define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
 #define TPCCLUS_MAX_NPADS  246u  /* 8 + npads + 2 columns must fit a 256-wide TMA box */
+#define TPCCLUS_MAX_PENDING 64    /* runs that may be enqueued before their tpcclus_result */
 #define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
 
 /* One zero-suppressed digit, 8 bytes (BASELINE.json:configs[0]: "uint8 row, uint8 pad,
@@ -138,15 +139,19 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
  *   d_out             DEVICE, out_capacity records, 16-byte aligned, owned by the caller.
  *                     Record k is the k-th peak in ascending (sector,row,time,pad) (D10).
  * At most one digit per cell is a precondition (D2); the result for duplicate cells is
- * unspecified but memory-safe.  One run in flight per context.
- * Errors (immediate): ERR_INVALID, ERR_CUDA.  Deferred to tpcclus_result: ERR_CAPACITY,
+ * unspecified but memory-safe.  Up to TPCCLUS_MAX_PENDING runs may be enqueued before their
+ * results are collected, all on the SAME stream (they share the charge map and execute in
+ * order; no host synchronisation is needed between the fragments of a time frame).
+ * Errors (immediate): ERR_INVALID (also: too many pending runs, or a different stream while
+ * runs are pending), ERR_CUDA.  Deferred to tpcclus_result: ERR_CAPACITY,
  * ERR_DIGIT, ERR_CUDA. */
 int tpcclus_run(tpcclus_ctx* ctx, const tpcclus_digit* d_digits, uint64_t n,
                 const uint64_t* h_sector_offsets,
                 uint32_t t_core_begin, uint32_t t_core_end,
                 tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
 
-/* Wait for the run enqueued by tpcclus_run and report it.  Returns stats->status. */
+/* Wait for the OLDEST unreported run (FIFO) and report it.  Returns stats->status;
+ * ERR_INVALID if no run is pending. */
 int tpcclus_result(tpcclus_ctx* ctx, tpcclus_run_stats* stats);
 
 /* Same operation with HOST buffers (pageable or pinned): copies the digits host->device,
@@ -167,6 +172,12 @@ int tpcclus_run_host(tpcclus_ctx* ctx, const tpcclus_digit* h_digits, uint64_t n
 int tpcclus_run_tf_host(tpcclus_ctx* ctx, const tpcclus_fragment* frags, uint32_t n_frags,
                         tpcclus_cluster* h_out, uint64_t out_capacity,
                         tpcclus_run_stats* stats /* HOST [n_frags] */);
+
+/* Per-kernel device timing (for the roofline figures of bench.py): while on, every run is
+ * bracketed with CUDA events on ITS stream around k_clear (S0), k_scatter (S1) and k_cluster
+ * (S2..S7); tpcclus_result adds the elapsed times up.  set_profiling(1) resets the sums. */
+int tpcclus_set_profiling(tpcclus_ctx* ctx, int on);
+int tpcclus_get_profile(const tpcclus_ctx* ctx, double kernel_ms[3] /* HOST out */, uint64_t* n_runs /* HOST out */);
 
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 uint64_t tpcclus_launch_count(const tpcclus_ctx* ctx);

@@ -35,7 +35,7 @@ CLUSTER_DTYPE = np.dtype([
 assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
 
 EXPORTS = ("tpcclus_create", "tpcclus_run", "tpcclus_result", "tpcclus_run_host", "tpcclus_run_tf_host",
-           "tpcclus_launch_count", "tpcclus_device_bytes", "tpcclus_destroy", "tpcclus_strerror")
+           "tpcclus_set_profiling", "tpcclus_get_profile", "tpcclus_launch_count", "tpcclus_device_bytes", "tpcclus_destroy", "tpcclus_strerror")
 
 
 class tpcclus_geometry(ctypes.Structure):
@@ -89,6 +89,10 @@ def lib():
             L.tpcclus_run_tf_host.restype = ctypes.c_int
             L.tpcclus_run_tf_host.argtypes = [vp, ctypes.POINTER(tpcclus_fragment), u32, vp, u64,
                                               ctypes.POINTER(tpcclus_run_stats)]
+            L.tpcclus_set_profiling.restype = ctypes.c_int
+            L.tpcclus_set_profiling.argtypes = [vp, ctypes.c_int]
+            L.tpcclus_get_profile.restype = ctypes.c_int
+            L.tpcclus_get_profile.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
             L.tpcclus_launch_count.restype = u64
             L.tpcclus_launch_count.argtypes = [vp]
             L.tpcclus_device_bytes.restype = u64
@@ -179,6 +183,22 @@ def tpcclus_run_tf_host(ctx, fragments, h_out_ptr, out_capacity, check=True):
     if check and rc != TPCCLUS_OK:
         raise TpcclusError(rc, "tpcclus_run_tf_host")
     return out
+
+
+def tpcclus_set_profiling(ctx, on: bool) -> None:
+    rc = lib().tpcclus_set_profiling(ctx, 1 if on else 0)
+    if rc != TPCCLUS_OK:
+        raise TpcclusError(rc, "tpcclus_set_profiling")
+
+
+def tpcclus_get_profile(ctx):
+    """-> ({"k_clear": ms, "k_scatter": ms, "k_cluster": ms} summed over runs, n_runs)."""
+    ms = (ctypes.c_double * 3)()
+    n = ctypes.c_uint64()
+    rc = lib().tpcclus_get_profile(ctx, ms, ctypes.byref(n))
+    if rc != TPCCLUS_OK:
+        raise TpcclusError(rc, "tpcclus_get_profile")
+    return dict(k_clear=ms[0], k_scatter=ms[1], k_cluster=ms[2]), int(n.value)
 
 
 def tpcclus_launch_count(ctx) -> int:

@@ -17,6 +17,8 @@
 
 using namespace tpcclus;
 
+constexpr int kRing = TPCCLUS_MAX_PENDING;
+
 static_assert(sizeof(tpcclus_digit) == 8, "digit is 8 bytes");
 static_assert(sizeof(tpcclus_cluster) == 32 && sizeof(tpcclus_cluster) == sizeof(ClusterRec), "cluster is 32 bytes");
 
@@ -44,12 +46,18 @@ struct tpcclus_ctx {
   CUtensorMap* d_tmaps = nullptr;
   unsigned long long* d_tile_state = nullptr;
   DevStatus* d_status = nullptr;
-  // pinned host
+  // pinned host ring: one status slot per pending run (results are reported in FIFO order)
   DevStatus* h_status = nullptr;
-  // last run
+  struct Pending { uint64_t n, cap; };
+  Pending pending[kRing];
+  cudaEvent_t ev_done[kRing] = {};
+  cudaEvent_t ev_prof[kRing][4] = {};   // around k_clear / k_scatter / k_cluster when profiling
+  bool slot_profiled[kRing] = {};
+  uint64_t head = 0, tail = 0;          // runs reported / runs enqueued
   cudaStream_t last_stream = nullptr;
-  bool run_pending = false;
-  uint64_t last_n = 0, last_cap = 0;
+  bool profiling = false;
+  double prof_ms[3] = {0, 0, 0};
+  uint64_t prof_runs = 0;
   int sticky = TPCCLUS_OK;
   int sticky_cuda = 0;
   // host staging (TPCCLUS_OPT_HOST_STAGING)
@@ -117,7 +125,11 @@ void tpcclus_destroy(tpcclus_ctx* c) {
   if (!c) return;
   cudaSetDevice(c->device);
   if (c->s_run) cudaStreamSynchronize(c->s_run);
-  if (c->last_stream || c->run_pending) cudaStreamSynchronize(c->last_stream);
+  if (c->tail != c->head) cudaStreamSynchronize(c->last_stream);
+  for (int i = 0; i < kRing; ++i) {
+    if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+    for (int k = 0; k < 4; ++k) if (c->ev_prof[i][k]) cudaEventDestroy(c->ev_prof[i][k]);
+  }
   cudaFree(c->d_map); cudaFree(c->d_rows); cudaFree(c->d_tmaps); cudaFree(c->d_tile_state); cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
   for (int i = 0; i < 2; ++i) {
@@ -191,7 +203,12 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if ((rc = dev_alloc(c, &c->d_tmaps, uint64_t(g->n_sectors) * g->n_rows * sizeof(CUtensorMap))) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_tile_state, uint64_t(c->max_tiles) * 8)) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_status, sizeof(DevStatus))) != TPCCLUS_OK) return fail(rc);
-  if (cudaMallocHost(reinterpret_cast<void**>(&c->h_status), sizeof(DevStatus)) != cudaSuccess) return fail(TPCCLUS_ERR_NOMEM);
+  if (cudaMallocHost(reinterpret_cast<void**>(&c->h_status), kRing * sizeof(DevStatus)) != cudaSuccess) return fail(TPCCLUS_ERR_NOMEM);
+  for (int i = 0; i < kRing; ++i) {
+    if (cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
+    for (int k = 0; k < 4; ++k)
+      if (cudaEventCreate(&c->ev_prof[i][k]) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
+  }
   if (cudaMemcpy(c->d_rows, c->rows.data(), g->n_rows * sizeof(RowInfo), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8) != cudaSuccess ||
       cudaMemset(c->d_status, 0, sizeof(DevStatus)) != cudaSuccess)
@@ -261,7 +278,13 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
   for (uint32_t s = 0; s < g.n_sectors; ++s)
     if (h_off[s + 1] < h_off[s]) return TPCCLUS_ERR_INVALID;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (c->tail - c->head >= uint64_t(kRing)) return TPCCLUS_ERR_INVALID;          // too many unreported runs
+  if (c->tail != c->head && st != c->last_stream) return TPCCLUS_ERR_INVALID;    // pending runs share one stream
   CK(c, cudaSetDevice(c->device));
+  const int slot = int(c->tail % kRing);
+  const bool prof = c->profiling;
+  c->slot_profiled[slot] = prof;
+  if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][0], st));
 
   const int32_t origin = int32_t(b) - int32_t(g.halo_bins);
   const uint32_t tiles_per_row = (e - b + kTileT - 1) / kTileT;
@@ -284,6 +307,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     k_clear<<<grid, 256, 0, st>>>(c->d_map, c->d_rows, g.n_rows, c->sec_elems, rows_used, c->d_status);
     c->launches++;
     debug_check(st, "k_clear");
+    if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][1], st));
   }
   // S1: scatter
   if (n) {
@@ -302,6 +326,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     c->launches++;
     debug_check(st, "k_scatter");
   }
+  if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][2], st));
   // S2..S7: fused tile kernel
   {
     ClusterParams cp;
@@ -328,40 +353,64 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     c->launches++;
     debug_check(st, "k_cluster");
   }
+  if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][3], st));
   CK(c, cudaGetLastError());
-  CK(c, cudaMemcpyAsync(c->h_status, c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));
+  CK(c, cudaMemcpyAsync(&c->h_status[slot], c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));
+  CK(c, cudaEventRecord(c->ev_done[slot], st));
   c->last_stream = st;
-  c->run_pending = true;
-  c->last_n = n;
-  c->last_cap = cap;
+  c->pending[slot].n = n;
+  c->pending[slot].cap = cap;
+  c->tail++;
   return TPCCLUS_OK;
 }
 
 int tpcclus_result(tpcclus_ctx* c, tpcclus_run_stats* stats) {
   if (!c || !stats) return TPCCLUS_ERR_INVALID;
   std::memset(stats, 0, sizeof(*stats));
-  if (!c->run_pending) { stats->status = TPCCLUS_ERR_INVALID; return TPCCLUS_ERR_INVALID; }
+  if (c->head == c->tail) { stats->status = TPCCLUS_ERR_INVALID; return TPCCLUS_ERR_INVALID; }
   cudaSetDevice(c->device);
-  cudaError_t e = cudaStreamSynchronize(c->last_stream);
-  c->run_pending = false;
-  stats->n_digits_in = c->last_n;
+  const int slot = int(c->head % kRing);
+  cudaError_t e = cudaEventSynchronize(c->ev_done[slot]);
+  c->head++;
+  stats->n_digits_in = c->pending[slot].n;
   if (e != cudaSuccess) {
     stats->status = TPCCLUS_ERR_CUDA;
     stats->cuda_error = int(e);
     return TPCCLUS_ERR_CUDA;
   }
-  stats->n_digits_dropped = c->h_status->n_dropped;
-  stats->n_clusters = c->h_status->n_clusters;
+  if (c->slot_profiled[slot]) {
+    for (int k = 0; k < 3; ++k) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, c->ev_prof[slot][k], c->ev_prof[slot][k + 1]) == cudaSuccess) c->prof_ms[k] += ms;
+    }
+    c->prof_runs++;
+  }
+  stats->n_digits_dropped = c->h_status[slot].n_dropped;
+  stats->n_clusters = c->h_status[slot].n_clusters;
   int rc = TPCCLUS_OK;
   if ((c->g.options & TPCCLUS_OPT_STRICT_DIGITS) && stats->n_digits_dropped) rc = TPCCLUS_ERR_DIGIT;
-  else if (stats->n_clusters > c->last_cap) rc = TPCCLUS_ERR_CAPACITY;
+  else if (stats->n_clusters > c->pending[slot].cap) rc = TPCCLUS_ERR_CAPACITY;
   stats->status = rc;
   return rc;
 }
 
+int tpcclus_set_profiling(tpcclus_ctx* c, int on) {
+  if (!c) return TPCCLUS_ERR_INVALID;
+  c->profiling = on != 0;
+  if (on) { c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0; c->prof_runs = 0; }
+  return TPCCLUS_OK;
+}
+
+int tpcclus_get_profile(const tpcclus_ctx* c, double kernel_ms[3], uint64_t* n_runs) {
+  if (!c || !kernel_ms || !n_runs) return TPCCLUS_ERR_INVALID;
+  for (int k = 0; k < 3; ++k) kernel_ms[k] = c->prof_ms[k];
+  *n_runs = c->prof_runs;
+  return TPCCLUS_OK;
+}
+
 int tpcclus_run_tf_host(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf, tpcclus_cluster* h_out,
                         uint64_t cap, tpcclus_run_stats* stats) {
-  if (!c || !fr || !stats || nf == 0 || (cap && !h_out)) return TPCCLUS_ERR_INVALID;
+  if (!c || !fr || !stats || nf == 0 || (cap && !h_out) || c->head != c->tail) return TPCCLUS_ERR_INVALID;
   if (!(c->g.options & TPCCLUS_OPT_HOST_STAGING)) return TPCCLUS_ERR_INVALID;
   for (uint32_t f = 0; f < nf; ++f)
     if (fr[f].n > c->g.max_digits || (fr[f].n && !fr[f].h_digits) || !fr[f].h_sector_offsets) return TPCCLUS_ERR_INVALID;
