@@ -298,16 +298,14 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (algorithmic bytes per launch / mean launch time) ----
     peak, peak_src = measured_peak_gbs()
-    cells_core = int(npads.astype(np.int64).sum()) * cfg.n_sectors * sum(x["e"] - x["b"] for x in tf)
-    rows_used = [min(cfg.core_bins + 2 * cfg.halo_bins,
-                     ((x["e"] - x["b"] + 127) // 128) * 128 + cfg.halo_bins + 5) for x in tf]
-    pitch_sum = int(((npads.astype(np.int64) + 7) // 8 * 8).sum())
-    cells_cleared = sum(pitch_sum * cfg.n_sectors * r for r in rows_used)
     nfr = len(tf)
+    # digits appended to the tile lists: every digit once, plus once more when it lies within
+    # 5 bins of a 128-bin tile seam (10/128 of the core bins)
+    dup = 1.0 + 10.0 / 128.0
     alg = {   # bytes per launch, DESIGN.md §6
-        "k_clear": 2.0 * cells_cleared / nfr,                     # store every cell of the used rows once
-        "k_scatter": (8.0 + 2.0) * n_dig / nfr,                   # read 8 B/digit, write 2 B/digit
-        "k_cluster": (2.0 * cells_core + 32.0 * n_cl) / nfr,      # read every core cell once, write every record
+        "k_init": 4.0 * cfg.n_sectors * cfg.n_rows * ((cfg.core_bins + 127) // 128),   # one counter per tile
+        "k_bin": (8.0 + 4.0 * dup) * n_dig / nfr,                 # read 8 B/digit, append 4 B per list entry
+        "k_tile": (4.0 * dup * n_dig + 32.0 * n_cl) / nfr,        # read every list entry once, write every record
     }
     kern = {}
     for k, ms_sum in prof.items():
@@ -362,10 +360,10 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "u16 charges, int32/int64 moments, f64 finish", "data": "synthetic",
+        "dtype": "u16", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "digits_per_step": n_dig, "clusters_per_step": n_cl,
-                   "l2": "inputs larger than L2 (digits %.1f GB per step, map %.1f GB per fragment)"
-                         % (n_dig * 8 / 1e9, 2.0 * cells_cleared / nfr / 1e9),
+                   "l2": "inputs larger than L2 (digits %.1f GB per step, %.1f GB per fragment)"
+                         % (n_dig * 8 / 1e9, n_dig * 8 / nfr / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clusters_per_sec": n_cl * world / (ms_step * 1e-3),
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),

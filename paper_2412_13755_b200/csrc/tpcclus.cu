@@ -1,10 +1,9 @@
 // tpcclus.cu — C-ABI of include/tpcclus.h on top of the sm_100a kernels in tpcclus_kernels.cuh.
 //
-// Host logic only: argument checks, geometry tables, TMA descriptors, launches, the
-// host-staging pipeline.  Every step of the path runs in the kernels.  The CUDA driver API is
-// reached through cudaGetDriverEntryPoint (cuTensorMapEncodeTiled), so the library links
-// against the static CUDA runtime only and loads on a box without a GPU driver (where
-// tpcclus_create then fails loudly with TPCCLUS_ERR_CUDA — there is no CPU fallback).
+// Host logic only: argument checks, geometry tables, launches, the host-staging pipeline.
+// Every step of the path runs in the kernels.  The library links against the static CUDA
+// runtime only and loads on a box without a GPU driver (where tpcclus_create then fails
+// loudly with TPCCLUS_ERR_CUDA — there is no CPU fallback).
 #include "../../include/tpcclus.h"
 #include "tpcclus_kernels.cuh"
 
@@ -22,28 +21,24 @@ constexpr int kRing = TPCCLUS_MAX_PENDING;
 static_assert(sizeof(tpcclus_digit) == 8, "digit is 8 bytes");
 static_assert(sizeof(tpcclus_cluster) == 32 && sizeof(tpcclus_cluster) == sizeof(ClusterRec), "cluster is 32 bytes");
 
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 struct tpcclus_ctx {
   tpcclus_geometry g{};
   std::vector<uint16_t> npads;
   std::vector<RowInfo> rows;
   int device = 0;
-  uint32_t H = 0;                 // map rows per (sector,row): max_core_bins + 2*halo_bins
-  uint64_t sec_elems = 0;         // map elements per sector
+  uint32_t tiles_per_row_max = 0; // bins laid out per (sector,row): ceil(max_core_bins / kTileT)
+  uint64_t sec_list_elems = 0;    // digit-list elements per sector
   uint32_t max_tiles = 0;
-  uint32_t tile_bytes_max = 0, bm_words = 0, smem_bytes = 0;
-  int cluster_grid = 0;           // persistent grid of k_cluster
+  uint32_t map_bytes_max = 0, bm_words = 0, smem_bytes = 0;
+  int tile_grid = 0;              // persistent grid of k_tile
   int n_sm = 0;
   uint32_t epoch = 0;
   uint64_t launches = 0;
   uint64_t dev_bytes = 0;
   // device
-  uint16_t* d_map = nullptr;
+  uint32_t* d_lists = nullptr;    // fixed-capacity digit bins, one per (sector,row,time-tile)
+  uint32_t* d_counts = nullptr;   // digits appended per bin in the current run
   RowInfo* d_rows = nullptr;
-  CUtensorMap* d_tmaps = nullptr;
   unsigned long long* d_tile_state = nullptr;
   DevStatus* d_status = nullptr;
   // pinned host ring: one status slot per pending run (results are reported in FIFO order)
@@ -51,7 +46,7 @@ struct tpcclus_ctx {
   struct Pending { uint64_t n, cap; };
   Pending pending[kRing];
   cudaEvent_t ev_done[kRing] = {};
-  cudaEvent_t ev_prof[kRing][4] = {};   // around k_clear / k_scatter / k_cluster when profiling
+  cudaEvent_t ev_prof[kRing][4] = {};   // around k_init / k_bin / k_tile when profiling
   bool slot_profiled[kRing] = {};
   uint64_t head = 0, tail = 0;          // runs reported / runs enqueued
   cudaStream_t last_stream = nullptr;
@@ -130,7 +125,7 @@ void tpcclus_destroy(tpcclus_ctx* c) {
     if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
     for (int k = 0; k < 4; ++k) if (c->ev_prof[i][k]) cudaEventDestroy(c->ev_prof[i][k]);
   }
-  cudaFree(c->d_map); cudaFree(c->d_rows); cudaFree(c->d_tmaps); cudaFree(c->d_tile_state); cudaFree(c->d_status);
+  cudaFree(c->d_lists); cudaFree(c->d_counts); cudaFree(c->d_rows); cudaFree(c->d_tile_state); cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
   for (int i = 0; i < 2; ++i) {
     cudaFree(c->d_stage_digits[i]); cudaFree(c->d_stage_out[i]);
@@ -170,37 +165,37 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (prop.major < 10) return fail(TPCCLUS_ERR_CUDA);       // TMA + sm_100a code only; no fallback
   c->n_sm = prop.multiProcessorCount;
 
-  // geometry tables
-  c->H = g->max_core_bins + 2 * g->halo_bins;
+  // geometry tables: one digit bin per (sector, row, 128-bin time tile), one slot per map cell
+  c->tiles_per_row_max = (g->max_core_bins + kTileT - 1) / kTileT;
+  const uint32_t bin_rows = std::min<uint32_t>(uint32_t(kBoxH), g->max_core_bins + 2 * g->halo_bins);
   c->rows.resize(g->n_rows);
   uint64_t off = 0;
-  uint32_t max_boxw = 0, max_npads = 0;
+  uint32_t max_W = 0, max_npads = 0;
   for (uint32_t r = 0; r < g->n_rows; ++r) {
     RowInfo& ri = c->rows[r];
     ri.npads = c->npads[r];
-    ri.pitch = uint16_t(roundup(ri.npads, 8));
-    ri.boxw = uint16_t(roundup(kPadHalo + ri.npads + kPadTail, 8));
-    ri.nwords = uint16_t((ri.npads + 1) / 2);
+    ri.W = uint16_t(roundup(ri.npads + 2 * kColOff, 8));
+    ri.cap = roundup(bin_rows * ri.npads, 4);
+    ri.pad_ = 0;
     if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
-    ri.map_off = uint32_t(off);
-    off += uint64_t(c->H) * ri.pitch;
-    max_boxw = std::max<uint32_t>(max_boxw, ri.boxw);
+    ri.list_off = uint32_t(off);
+    off += uint64_t(c->tiles_per_row_max) * ri.cap;
+    max_W = std::max<uint32_t>(max_W, ri.W);
     max_npads = std::max<uint32_t>(max_npads, ri.npads);
   }
-  c->sec_elems = off;
-  c->tile_bytes_max = roundup(uint32_t(kBoxH) * max_boxw * 2u, 128);
+  c->sec_list_elems = off;
   c->bm_words = (max_npads + 8 + 31) / 32 + 1;
-  const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * ((g->max_core_bins + kTileT - 1) / kTileT);
-  if (tiles > 0x7FFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
+  c->map_bytes_max = roundup(uint32_t(kBoxH) * max_W * 2u + uint32_t(kBoxH) * c->bm_words * 4u, 16);
+  const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * c->tiles_per_row_max;
+  if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
-  c->smem_bytes = kStages * c->tile_bytes_max + 16 * 8 + 16 * 4 + 16 * 4 + kListCap * 4 + 256 * sizeof(RowInfo) +
-                  (kTileT + 4) * 4 + kBoxH * c->bm_words * 4 + 128;
+  c->smem_bytes = kDigCap * 4 + c->map_bytes_max + 16 + 16 + 16 * 4 + kListCap * 4 + (kTileT + 4) * 4 + 128;
 
   int rc;
-  const uint64_t map_bytes = uint64_t(g->n_sectors) * c->sec_elems * 2;
-  if ((rc = dev_alloc(c, &c->d_map, map_bytes)) != TPCCLUS_OK) return fail(rc);
+  const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;
+  if ((rc = dev_alloc(c, &c->d_lists, list_bytes)) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_counts, (uint64_t(c->max_tiles) + 4) * 4)) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_rows, g->n_rows * sizeof(RowInfo))) != TPCCLUS_OK) return fail(rc);
-  if ((rc = dev_alloc(c, &c->d_tmaps, uint64_t(g->n_sectors) * g->n_rows * sizeof(CUtensorMap))) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_tile_state, uint64_t(c->max_tiles) * 8)) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_status, sizeof(DevStatus))) != TPCCLUS_OK) return fail(rc);
   if (cudaMallocHost(reinterpret_cast<void**>(&c->h_status), kRing * sizeof(DevStatus)) != cudaSuccess) return fail(TPCCLUS_ERR_NOMEM);
@@ -214,40 +209,12 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
       cudaMemset(c->d_status, 0, sizeof(DevStatus)) != cudaSuccess)
     return fail(TPCCLUS_ERR_CUDA);
 
-  // one 2-D TMA descriptor per (sector,row): dims {npads, H}, row stride pitch*2 bytes,
-  // box {boxw, kBoxH}; out-of-range box elements are zero-filled (D2)
-  {
-    PFN_encodeTiled encode = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    void* fn = nullptr;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
-        qres != cudaDriverEntryPointSuccess || !fn)
-      return fail(TPCCLUS_ERR_CUDA);
-    encode = reinterpret_cast<PFN_encodeTiled>(fn);
-    std::vector<CUtensorMap> maps(size_t(g->n_sectors) * g->n_rows);
-    for (uint32_t s = 0; s < g->n_sectors; ++s)
-      for (uint32_t r = 0; r < g->n_rows; ++r) {
-        const RowInfo& ri = c->rows[r];
-        cuuint64_t gdim[2] = {ri.npads, c->H};
-        cuuint64_t gstr[1] = {cuuint64_t(ri.pitch) * 2};
-        cuuint32_t box[2] = {ri.boxw, cuuint32_t(kBoxH)};
-        cuuint32_t estr[2] = {1, 1};
-        void* base = c->d_map + uint64_t(s) * c->sec_elems + ri.map_off;
-        CUresult cr = encode(&maps[size_t(s) * g->n_rows + r], CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, base, gdim, gstr,
-                             box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (cr != CUDA_SUCCESS) return fail(TPCCLUS_ERR_CUDA);
-      }
-    if (cudaMemcpy(c->d_tmaps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess)
-      return fail(TPCCLUS_ERR_CUDA);
-  }
-
-  if (cudaFuncSetAttribute(k_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, int(c->smem_bytes)) != cudaSuccess)
+  if (cudaFuncSetAttribute(k_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, int(c->smem_bytes)) != cudaSuccess)
     return fail(TPCCLUS_ERR_CUDA);
   int occ = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_cluster, kThreads, c->smem_bytes) != cudaSuccess || occ < 1)
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tile, kThreads, c->smem_bytes) != cudaSuccess || occ < 1)
     return fail(TPCCLUS_ERR_CUDA);
-  c->cluster_grid = occ * c->n_sm;
+  c->tile_grid = occ * c->n_sm;
 
   if (g->options & TPCCLUS_OPT_HOST_STAGING) {
     for (int i = 0; i < 2; ++i) {
@@ -286,72 +253,70 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
   c->slot_profiled[slot] = prof;
   if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][0], st));
 
-  const int32_t origin = int32_t(b) - int32_t(g.halo_bins);
   const uint32_t tiles_per_row = (e - b + kTileT - 1) / kTileT;
   const uint32_t n_tiles = g.n_sectors * g.n_rows * tiles_per_row;
-  // rows of the map that a TMA box of this run can touch (rows >= H are zero-filled by TMA)
-  const uint32_t rows_used = std::min<uint32_t>(c->H, tiles_per_row * kTileT + g.halo_bins + kReach);
   c->epoch = (c->epoch + 1) & 0x3FFFFFFFu;
   if (c->epoch == 0) {   // wrapped: stale words could alias, so wipe them once
     CK(c, cudaMemsetAsync(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8, st));
     c->epoch = 1;
   }
 
-  // S0: clear
+  // S0: counters + status
   {
-    uint32_t max_pitch = 0;
-    for (const RowInfo& ri : c->rows) max_pitch = std::max<uint32_t>(max_pitch, ri.pitch);
-    const uint64_t span16 = (uint64_t(rows_used) * max_pitch) >> 3;
-    const uint32_t chunks = uint32_t(std::min<uint64_t>(std::max<uint64_t>((span16 + 256 * 8 - 1) / (256 * 8), 1), 65535));
-    dim3 grid(g.n_sectors * g.n_rows, chunks);
-    k_clear<<<grid, 256, 0, st>>>(c->d_map, c->d_rows, g.n_rows, c->sec_elems, rows_used, c->d_status);
+    const uint32_t blocks = std::min<uint32_t>((n_tiles / 4 + 256) / 256, uint32_t(c->n_sm) * 8);
+    k_init<<<std::max(blocks, 1u), 256, 0, st>>>(c->d_counts, n_tiles, c->d_status);
     c->launches++;
-    debug_check(st, "k_clear");
+    debug_check(st, "k_init");
     if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][1], st));
   }
-  // S1: scatter
+  // S1: binning
   if (n) {
-    ScatterParams sp;
-    sp.n = n;
-    sp.sec_elems = c->sec_elems;
-    sp.t_origin = origin;
-    sp.t_lo = std::max<int32_t>(0, origin);
-    sp.t_hi = int32_t(std::min<uint64_t>(g.tf_time_bins, uint64_t(e) + g.halo_bins));
-    sp.n_sectors = g.n_sectors;
-    sp.n_rows = g.n_rows;
-    std::memcpy(sp.off, h_off, (g.n_sectors + 1) * sizeof(uint64_t));
+    BinParams bp;
+    bp.n = n;
+    bp.sec_list_elems = c->sec_list_elems;
+    bp.t_core_begin = int32_t(b);
+    bp.t_lo = std::max<int32_t>(0, int32_t(b) - int32_t(g.halo_bins));
+    bp.t_hi = int32_t(std::min<uint64_t>(g.tf_time_bins, uint64_t(e) + g.halo_bins));
+    bp.n_sectors = g.n_sectors;
+    bp.n_rows = g.n_rows;
+    bp.tiles_per_row = tiles_per_row;
+    bp.tiles_per_row_max = c->tiles_per_row_max;
+    std::memcpy(bp.off, h_off, (g.n_sectors + 1) * sizeof(uint64_t));
     const uint64_t pairs = (n + 1) / 2;
     const uint32_t blocks = uint32_t(std::min<uint64_t>((pairs + 255) / 256, uint64_t(c->n_sm) * 16));
-    k_scatter<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), sp, c->d_rows, c->d_map, c->d_status);
+    k_bin<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), bp, c->d_rows, c->d_lists,
+                                                c->d_counts, c->d_status);
     c->launches++;
-    debug_check(st, "k_scatter");
+    debug_check(st, "k_bin");
   }
   if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][2], st));
-  // S2..S7: fused tile kernel
+  // S1..S7: fused tile kernel
   {
-    ClusterParams cp;
-    cp.tmaps = c->d_tmaps;
-    cp.rows = c->d_rows;
-    cp.tile_state = c->d_tile_state;
-    cp.status = c->d_status;
-    cp.out = d_out;
-    cp.out_capacity = cap;
-    cp.n_sectors = g.n_sectors;
-    cp.n_rows = g.n_rows;
-    cp.tiles_per_row = tiles_per_row;
-    cp.n_tiles = n_tiles;
-    cp.t_core_begin = int32_t(b);
-    cp.t_core_end = int32_t(e);
-    cp.t_origin = origin;
-    cp.tf_time_bins = g.tf_time_bins;
-    cp.theta = g.peak_min_q16;
-    cp.epoch = c->epoch;
-    cp.tile_bytes_max = c->tile_bytes_max;
-    cp.bm_words = c->bm_words;
-    const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->cluster_grid)));
-    k_cluster<<<grid, kThreads, c->smem_bytes, st>>>(cp);
+    TileParams tp;
+    tp.rows = c->d_rows;
+    tp.lists = c->d_lists;
+    tp.counts = c->d_counts;
+    tp.tile_state = c->d_tile_state;
+    tp.status = c->d_status;
+    tp.out = d_out;
+    tp.out_capacity = cap;
+    tp.sec_list_elems = c->sec_list_elems;
+    tp.n_sectors = g.n_sectors;
+    tp.n_rows = g.n_rows;
+    tp.tiles_per_row = tiles_per_row;
+    tp.tiles_per_row_max = c->tiles_per_row_max;
+    tp.n_tiles = n_tiles;
+    tp.t_core_begin = int32_t(b);
+    tp.t_core_end = int32_t(e);
+    tp.tf_time_bins = g.tf_time_bins;
+    tp.theta = g.peak_min_q16;
+    tp.epoch = c->epoch;
+    tp.map_bytes_max = c->map_bytes_max;
+    tp.bm_words = c->bm_words;
+    const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->tile_grid)));
+    k_tile<<<grid, kThreads, c->smem_bytes, st>>>(tp);
     c->launches++;
-    debug_check(st, "k_cluster");
+    debug_check(st, "k_tile");
   }
   if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][3], st));
   CK(c, cudaGetLastError());

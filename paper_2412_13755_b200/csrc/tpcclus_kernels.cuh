@@ -1,15 +1,20 @@
 // tpcclus_kernels.cuh — sm_100a kernels of the TPC cluster finder (device side).
 //
-// Steps of SURVEY.md §8(a) and where they run:
-//   S0  map clear            k_clear      (HBM store-only)
-//   S1  charge-map fill      k_scatter    (16-byte digit loads, 2-byte scattered stores)
-//   S2  peak finding         k_cluster    phase A: TMA tile (+halo) -> smem, packed u16x2 3x3 ordered max
-//   S3  peak count S(c)      k_cluster    phase C: 9x9 flag window from the smem flag bitmap
-//   S4  5x5 assembly         k_cluster    phase C: one thread per peak, 25 charges from the smem tile
-//   S5  centroid / width     k_cluster    phase C: exact integer moments, fp64 finish
-//   S6  ordered compaction   k_cluster    phase B: popc prefix inside the tile + decoupled look-back
-//                                         across tiles in (sector,row,time) ticket order
-//   S7  fragment ownership   k_cluster    tiles cover exactly the core [b,e); halo rows are only read
+// Steps of SURVEY.md §8(a) and where they run (DESIGN.md §5):
+//   S0  set-up               k_init   zero the per-tile digit counters and the run status
+//   S1  charge-map fill      k_bin    16-byte digit loads, D1 quantisation, digit -> packed 4-byte
+//                                     record appended to the list of every (sector,row,time-tile)
+//                                     whose window holds it (tile halo duplicated here)
+//                            k_tile   the tile's list is staged in shared memory by a TMA bulk copy
+//                                     and scattered into the (pad x time) charge map of the tile,
+//                                     which lives in shared memory only
+//   S2  peak finding         k_tile   digit-driven 3x3 ordered-maximum test on the smem map -> flag bitmap
+//   S3  peak count S(c)      k_tile   9x9 flag window from the smem flag bitmap
+//   S4  5x5 assembly         k_tile   one thread per peak, charges from the smem map
+//   S5  centroid / width     k_tile   exact integer moments, fp64 finish
+//   S6  ordered compaction   k_tile   popc prefix inside the tile + decoupled look-back across tiles
+//                                     in (sector,row,time) ticket order, by a dedicated warp
+//   S7  fragment ownership   k_tile   tiles cover exactly the core [b,e); halo rows never emit
 //
 // Definitions D1..D12 are those of SURVEY.md §8(c) (restated in DESIGN.md §2); the D-number
 // is cited where each rule is implemented.  No code here is shared with oracle/.
@@ -20,63 +25,66 @@
 
 namespace tpcclus {
 
-constexpr int      kThreads      = 256;   // CTA size of k_cluster
+constexpr int      kThreads      = 256;   // CTA size of k_tile
+constexpr int      kBuildThreads = 224;   // warps 0..6 build clusters; warp 7 prefetches and looks back
 constexpr int      kTileT        = 128;   // core time bins per tile
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
-constexpr int      kBoxH         = kTileT + 2 * kReach;   // tile rows staged in smem
-constexpr int      kPadHalo      = 8;     // box starts at pad -8: the innermost TMA coordinate must be a multiple
-                                          // of 16 bytes (measured: -2 raises 'illegal instruction'); 2 would do for 5x5
-constexpr int      kPadTail      = 2;     // cells kept right of the last pad (5x5 window)
-constexpr int      kStages       = 2;     // TMA double buffering
+constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
+constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
 constexpr int      kListCap      = 1024;  // peaks processed per pass inside one tile
+constexpr int      kDigCap       = 4096;  // digits staged per TMA bulk copy (16 KB)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 
 struct RowInfo {              // one per pad row (device table)
-  uint32_t map_off;           // element offset of this row's [H][pitch] block inside one sector's map
+  uint32_t list_off;          // element offset of this row's bins inside one sector's digit lists
+  uint32_t cap;               // list capacity of one bin = roundup4(map rows * npads): one slot per cell
   uint16_t npads;
-  uint16_t pitch;             // elements, multiple of 8 (TMA: global stride multiple of 16 bytes)
-  uint16_t boxw;              // TMA box width in elements = roundup8(kPadHalo + npads + kPadTail)
-  uint16_t nwords;            // active 2-cell word columns = ceil(npads/2)
+  uint16_t W;                 // smem map pitch in cells = roundup8(npads + 4)
+  uint32_t pad_;
 };
 
 struct DevStatus {            // device-side run status, copied to pinned host memory after the run
   unsigned long long n_dropped;
   unsigned long long n_clusters;
-  unsigned int       ticket;  // tile ticket counter of k_cluster
+  unsigned int       ticket;  // tile ticket counter of k_tile
   unsigned int       pad_;
 };
 
-struct ScatterParams {
+struct BinParams {
   uint64_t n;                          // digits
-  uint64_t sec_elems;                  // map elements per sector
-  int32_t  t_origin;                   // global time of local map row 0 (= b - halo, may be negative)
-  int32_t  t_lo, t_hi;                 // loaded range [lo,hi) in global time
+  uint64_t sec_list_elems;             // list elements per sector
+  int32_t  t_core_begin;               // b
+  int32_t  t_lo, t_hi;                 // loaded range [lo,hi) in global time (D1)
   uint32_t n_sectors, n_rows;
+  uint32_t tiles_per_row;              // tiles of this run
+  uint32_t tiles_per_row_max;          // bins laid out per (sector,row)
   uint64_t off[kMaxSectors + 1];       // sector offsets (copied from the host array)
 };
 
-struct ClusterParams {
-  const CUtensorMap* tmaps;            // [n_sectors*n_rows], global memory
+struct TileParams {
   const RowInfo*     rows;             // [n_rows]
+  const uint32_t*    lists;            // packed digits, fixed-capacity bins
+  const uint32_t*    counts;           // [n_tiles] digits appended per bin (may exceed cap: clamp)
   unsigned long long* tile_state;      // [n_tiles] decoupled look-back words
   DevStatus*         status;
   void*              out;              // tpcclus_cluster records
   uint64_t           out_capacity;
+  uint64_t           sec_list_elems;
   uint32_t n_sectors, n_rows;
   uint32_t tiles_per_row;              // ceil((e-b)/kTileT)
+  uint32_t tiles_per_row_max;
   uint32_t n_tiles;
   int32_t  t_core_begin, t_core_end;   // [b,e)
-  int32_t  t_origin;                   // global time of local map row 0
   uint32_t tf_time_bins;
   uint32_t theta;                      // peak_min_q16
   uint32_t epoch;                      // run counter, tags tile_state words
-  uint32_t tile_bytes_max;             // smem bytes reserved per stage
+  uint32_t map_bytes_max;              // smem bytes reserved for map + flag bitmap
   uint32_t bm_words;                   // flag-bitmap words per tile row
 };
 
 // ----------------------------------------------------------------------------------------
-// small PTX wrappers (TMA + mbarrier), sm_90+/sm_100a
+// small PTX wrappers (TMA bulk copy + mbarrier), sm_90+/sm_100a
 // ----------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -104,21 +112,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
-// 2-D tiled TMA load global -> shared; out-of-range coordinates are zero-filled, which is
-// exactly D2's "0 for every out-of-range pad or time".
-__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, int x, int y,
-                                            uint64_t* bar) {
+// 1-D TMA bulk copy global -> shared (UBLKCP): 16-byte aligned addresses, size a multiple of 16.
+__device__ __forceinline__ void tma_bulk_load(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
   asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
           "r"(smem_u32(smem_dst)),
-      "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(x), "r"(y)
+      "l"(reinterpret_cast<uint64_t>(gsrc)), "r"(bytes), "r"(smem_u32(bar))
       : "memory");
 }
-// The descriptors live in global memory (written once by the host in tpcclus_create); make them
-// visible to the tensormap proxy of this SM before the first TMA that uses them.
-__device__ __forceinline__ void tensormap_fence_acquire(const CUtensorMap* tmap) {
-  asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(reinterpret_cast<uint64_t>(tmap))
-               : "memory");
+__device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
   unsigned long long v;
@@ -137,31 +140,29 @@ __device__ __forceinline__ uint4 ld_stream_u4(const uint4* p) {   // streaming 1
 }
 
 // ----------------------------------------------------------------------------------------
-// S0: clear the rows of the charge map that this run can read or write.
-// grid = (n_sectors*n_rows, chunks); each (sector,row) block [rows_used][pitch] is contiguous.
+// S0: zero the per-tile digit counters of this run and the run status.
 // ----------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_clear(uint16_t* __restrict__ map, const RowInfo* __restrict__ rows,
-                                               uint32_t n_rows, uint64_t sec_elems, uint32_t rows_used,
-                                               DevStatus* __restrict__ status) {
-  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) {
+__global__ void __launch_bounds__(256) k_init(uint32_t* __restrict__ counts, uint32_t n_tiles,
+                                              DevStatus* __restrict__ status) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) {
     status->n_dropped = 0ull;
     status->n_clusters = 0ull;
     status->ticket = 0u;
   }
-  const uint32_t sr = blockIdx.x;
-  const uint32_t s = sr / n_rows, r = sr - s * n_rows;
-  const RowInfo ri = rows[r];
-  const uint64_t span16 = (uint64_t(rows_used) * ri.pitch) >> 3;       // 16-byte units (pitch % 8 == 0)
-  uint4* base = reinterpret_cast<uint4*>(map + uint64_t(s) * sec_elems + ri.map_off);
-  const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-  for (uint64_t i = uint64_t(blockIdx.y) * blockDim.x + threadIdx.x; i < span16;
-       i += uint64_t(gridDim.y) * blockDim.x)
-    base[i] = z;
+  const uint32_t n4 = (n_tiles + 3u) >> 2;                 // the array is padded to a multiple of 4
+  for (uint32_t k = i; k < n4; k += gridDim.x * blockDim.x)
+    reinterpret_cast<uint4*>(counts)[k] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 // ----------------------------------------------------------------------------------------
-// S1: digit scatter.  One 16-byte load = two digits (BASELINE.json:north_star (2): "16-byte
-// vectorised coalesced loads").  D1 quantisation, D2 map fill, invalid digits dropped+counted.
+// S1 (first half): digit binning.  One 16-byte load = two digits (BASELINE.json:north_star (2):
+// "16-byte vectorised coalesced loads").  D1 quantisation; invalid digits dropped and counted.
+// A valid digit at global time t is appended, as pad | tl<<8 | q16<<16 with tl its row inside
+// the tile's 138-row window, to the list of every tile tt whose window
+// [b + 128 tt - 5, b + 128 tt + 133) contains t (one tile, or two next to a tile seam).
+// A bin has one slot per map cell, so it cannot overflow while D2's precondition (at most one
+// digit per cell) holds; slots past the capacity are discarded (memory-safe for duplicates).
 // ----------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t quantise_q16(float charge) {
   // D1: q16 = clamp(rint(charge*16), 0, 16368); rint = round-half-even (cvt.rni); NaN -> 0
@@ -170,9 +171,9 @@ __device__ __forceinline__ uint32_t quantise_q16(float charge) {
   return x >= float(kQClamp) ? kQClamp : uint32_t(x);
 }
 
-__device__ __forceinline__ bool scatter_one(uint32_t w0, uint32_t w1, uint64_t idx, uint32_t& sector,
-                                            const ScatterParams& P, const RowInfo* srow,
-                                            uint16_t* __restrict__ map) {
+__device__ __forceinline__ bool bin_one(uint32_t w0, uint32_t w1, uint64_t idx, uint32_t& sector,
+                                        const BinParams& P, const RowInfo* srow, uint32_t* __restrict__ lists,
+                                        uint32_t* __restrict__ counts) {
   while (idx >= P.off[sector + 1]) ++sector;     // digits are grouped per sector; rarely iterates
   const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
   const int32_t time = int32_t(w0 >> 16);
@@ -180,14 +181,24 @@ __device__ __forceinline__ bool scatter_one(uint32_t w0, uint32_t w1, uint64_t i
   if (q == 0u || row >= P.n_rows || time < P.t_lo || time >= P.t_hi) return false;
   const RowInfo ri = srow[row];
   if (pad >= ri.npads) return false;
-  const uint64_t e = uint64_t(sector) * P.sec_elems + ri.map_off + uint64_t(time - P.t_origin) * ri.pitch + pad;
-  map[e] = uint16_t(q);
+  const int32_t u = time - P.t_core_begin;                       // >= -halo
+  int32_t tt_hi = (u + kReach) >> 7;                             // largest tt with 128 tt - 5 <= u
+  int32_t tt_lo = ((u - (kTileT + kReach)) >> 7) + 1;            // smallest tt with u < 128 tt + 133
+  tt_lo = max(tt_lo, 0);
+  tt_hi = min(tt_hi, int32_t(P.tiles_per_row) - 1);
+  const uint32_t sr = sector * P.n_rows + row;
+  const uint64_t base = uint64_t(sector) * P.sec_list_elems + ri.list_off;
+  for (int32_t tt = tt_lo; tt <= tt_hi; ++tt) {
+    const uint32_t tl = uint32_t(u - tt * kTileT + kReach);      // 0..137
+    const uint32_t slot = atomicAdd(&counts[sr * P.tiles_per_row + uint32_t(tt)], 1u);
+    if (slot < ri.cap) lists[base + uint64_t(tt) * ri.cap + slot] = pad | (tl << 8) | (q << 16);
+  }
   return true;
 }
 
-__global__ void __launch_bounds__(256) k_scatter(const uint2* __restrict__ digits, const __grid_constant__ ScatterParams P,
-                                                 const RowInfo* __restrict__ rows, uint16_t* __restrict__ map,
-                                                 DevStatus* __restrict__ status) {
+__global__ void __launch_bounds__(256) k_bin(const uint2* __restrict__ digits, const __grid_constant__ BinParams P,
+                                             const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
+                                             uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
   __shared__ RowInfo srow[256];
   for (uint32_t i = threadIdx.x; i < P.n_rows; i += blockDim.x) srow[i] = rows[i];
   __syncthreads();
@@ -214,14 +225,14 @@ __global__ void __launch_bounds__(256) k_scatter(const uint2* __restrict__ digit
   for (uint64_t i = tid; i < npairs; i += stride) {
     const uint4 v = ld_stream_u4(pairs + i);
     const uint64_t idx = head + 2 * i;
-    dropped += scatter_one(v.x, v.y, idx, sector, P, srow, map) ? 0u : 1u;
-    dropped += scatter_one(v.z, v.w, idx + 1, sector, P, srow, map) ? 0u : 1u;
+    dropped += bin_one(v.x, v.y, idx, sector, P, srow, lists, counts) ? 0u : 1u;
+    dropped += bin_one(v.z, v.w, idx + 1, sector, P, srow, lists, counts) ? 0u : 1u;
   }
   if (tid == 0) {                                 // leftovers: the peeled head and an odd tail
     uint32_t s0 = 0;
-    if (head && n > 0) dropped += scatter_one(digits[0].x, digits[0].y, 0, s0, P, srow, map) ? 0u : 1u;
+    if (head && n > 0) dropped += bin_one(digits[0].x, digits[0].y, 0, s0, P, srow, lists, counts) ? 0u : 1u;
     const uint64_t tail = head + 2 * npairs;
-    if (tail < n) dropped += scatter_one(digits[tail].x, digits[tail].y, tail, s0, P, srow, map) ? 0u : 1u;
+    if (tail < n) dropped += bin_one(digits[tail].x, digits[tail].y, tail, s0, P, srow, lists, counts) ? 0u : 1u;
   }
   // warp-aggregated count of dropped digits
   dropped = __reduce_add_sync(0xffffffffu, dropped);
@@ -229,7 +240,7 @@ __global__ void __launch_bounds__(256) k_scatter(const uint2* __restrict__ digit
 }
 
 // ----------------------------------------------------------------------------------------
-// S2..S7: fused tile kernel.
+// S1 (second half) .. S7: fused tile kernel.
 // ----------------------------------------------------------------------------------------
 struct __align__(16) ClusterRec {   // byte-for-byte the tpcclus_cluster of include/tpcclus.h
   uint32_t w0;                      // sector | row<<8 | pad<<16 | flags<<24
@@ -282,19 +293,19 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
 
 __device__ __constant__ uint16_t kShareWeight[10] = {0, 2520, 1260, 840, 630, 504, 420, 360, 315, 280};  // D6: L/S
 
-// One thread builds one cluster (S3..S5).  tile: smem charges [kBoxH][boxw]; bm: smem flag
-// bitmap [kBoxH][bmw], bit (pad+4) of row j set iff the cell is a peak (D4).
-__device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile, const uint32_t* __restrict__ bm,
-                                              uint32_t boxw, uint32_t bmw, uint32_t j, uint32_t pad,
+// One thread builds one cluster (S3..S5).  map: smem charges [kBoxH][W], column = pad + kColOff;
+// bm: smem flag bitmap [kBoxH][bmw], bit (pad+4) of row j set iff the cell is a peak (D4).
+__device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ map, const uint32_t* __restrict__ bm,
+                                              uint32_t W, uint32_t bmw, uint32_t j, uint32_t pad,
                                               uint32_t sector, uint32_t row, uint32_t npads, int32_t tglob,
                                               uint32_t tf_time_bins, ClusterRec& rec) {
-  // 5x5 charges around the peak: box column of pad p is p + kPadHalo
+  // 5x5 charges around the peak: map column of pad p is p + kColOff
   uint32_t q[5][5];
-  const uint16_t* c0 = tile + (j - 2) * boxw + (pad + kPadHalo - 2);
+  const uint16_t* c0 = map + (j - 2) * W + (pad + kColOff - 2);
 #pragma unroll
   for (int dt = 0; dt < 5; ++dt)
 #pragma unroll
-    for (int dp = 0; dp < 5; ++dp) q[dt][dp] = c0[dt * boxw + dp];
+    for (int dp = 0; dp < 5; ++dp) q[dt][dp] = c0[dt * W + dp];
 
   // 9x9 peak-flag window: F[k] bit i  <->  row j-4+k, pad  p-4+i  (bitmap bit = pad + 4)
   uint32_t F[9];
@@ -310,7 +321,7 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
   }
 
   const uint32_t qP = q[2][2];
-  uint32_t W = qP * 2520u, Mpp = 0, Mtt = 0, ncells = 1, flags = 0;
+  uint32_t W_ = qP * 2520u, Mpp = 0, Mtt = 0, ncells = 1, flags = 0;
   int32_t Mp = 0, Mt = 0;
   if (qP == kQClamp) flags |= 4u;
 #pragma unroll
@@ -344,7 +355,7 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
           for (int jt = -2; jt <= 2; ++jt) S += __popc((F[dt + jt + 4] >> (dp + 2)) & 0x1Fu);
         }
         const uint32_t w = qc * uint32_t(kShareWeight[S]);     // D6 weight in 1/(16*2520) ADC
-        W += w;                                                // D7 moments, exact integers
+        W_ += w;                                               // D7 moments, exact integers
         Mp += int32_t(w) * dp;
         Mt += int32_t(w) * dt;
         Mpp += w * uint32_t(dp * dp);
@@ -357,9 +368,9 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
   if (pad < 2u || pad + 2u >= npads) flags |= 1u;              // D8 EDGE_PAD
   if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
   // D8: evaluated in double from the exact integers, rounded once to float32
-  const double Wd = double(W);
-  const long long Np = (long long)Mpp * (long long)W - (long long)Mp * (long long)Mp;
-  const long long Nt = (long long)Mtt * (long long)W - (long long)Mt * (long long)Mt;
+  const double Wd = double(W_);
+  const long long Np = (long long)Mpp * (long long)W_ - (long long)Mp * (long long)Mp;
+  const long long Nt = (long long)Mtt * (long long)W_ - (long long)Mt * (long long)Mt;
   rec.w0 = sector | (row << 8) | (pad << 16) | (flags << 24);
   rec.time = uint32_t(tglob);
   rec.w2 = qP | (ncells << 16);
@@ -370,128 +381,151 @@ __device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ tile,
   rec.sigma_time = float(sqrt(double(Nt)) / Wd);
 }
 
-__global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__ ClusterParams P) {
+__device__ __forceinline__ void store_rec(void* out, uint64_t g, const ClusterRec& rec) {
+  uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<ClusterRec*>(out) + g);
+  const uint4* s4 = reinterpret_cast<const uint4*>(&rec);
+  o[0] = s4[0];
+  o[1] = s4[1];
+}
+
+// D4 on the smem map for the digit (pad, tl, q): strictly greater than the 4 neighbours earlier
+// in (time,pad) order, >= the 4 later ones.  map32: the map as 32-bit words (two cells).
+__device__ __forceinline__ bool is_peak(const uint32_t* __restrict__ map32, uint32_t wpr, uint32_t pad, uint32_t tl,
+                                        uint32_t q) {
+  const uint32_t c = pad + kColOff;
+  const uint32_t sh = (c & 1u) ? 0u : 16u;                      // cells c-1,c,c+1 start at bit sh of (w0,w1)
+  const uint32_t* r = map32 + tl * wpr + ((c - 1u) >> 1);
+  const uint32_t a0 = r[-int32_t(wpr)], a1 = r[1 - int32_t(wpr)];
+  const uint32_t b0 = r[0], b1 = r[1];
+  const uint32_t c0 = r[wpr], c1 = r[wpr + 1];
+  const uint32_t A = __funnelshift_r(a0, a1, sh), Ar = (a1 >> sh) & 0xFFFFu;   // A = left | centre<<16
+  const uint32_t B = __funnelshift_r(b0, b1, sh), Br = (b1 >> sh) & 0xFFFFu;
+  const uint32_t C = __funnelshift_r(c0, c1, sh), Cr = (c1 >> sh) & 0xFFFFu;
+  const uint32_t early = max(max(A & 0xFFFFu, A >> 16), max(Ar, B & 0xFFFFu));
+  const uint32_t late = max(max(C & 0xFFFFu, C >> 16), max(Cr, Br));
+  return q > early && q >= late;
+}
+
+__global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ TileParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
-  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // TMA destination: 128-byte aligned
-  uint16_t* tile_buf[kStages];
-#pragma unroll
-  for (int s = 0; s < kStages; ++s) { tile_buf[s] = reinterpret_cast<uint16_t*>(sp); sp += P.tile_bytes_max; }
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += 16 * 8;        // kStages used, keeps 128-byte alignment
-  uint32_t* s_tile = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // tile id per stage
+  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  uint32_t* lbuf = reinterpret_cast<uint32_t*>(sp);         sp += kDigCap * 4;   // TMA bulk destination
+  uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += 16;
+  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // [0] tile, [1] digits (next tile)
   uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // [0] exclusive prefix, [1..8] warp totals
   uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
-  RowInfo* srow = reinterpret_cast<RowInfo*>(sp);           sp += 256 * sizeof(RowInfo);
   uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
-  uint32_t* bm = reinterpret_cast<uint32_t*>(sp);
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  for (uint32_t i = tid; i < P.n_rows; i += kThreads) srow[i] = P.rows[i];
+  const uint32_t bmw = P.bm_words;
   if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) mbar_init(&mbar[s], 1);
+    mbar_init(mbar, 1);
     fence_mbar_init();
   }
   __syncthreads();
 
-  // issue the TMA load of the next ticketed tile into stage s (thread 0 only)
-  auto fetch = [&](int s) {
-    const uint32_t t = atomicAdd(&P.status->ticket, 1u);
-    s_tile[s] = t;
-    if (t < P.n_tiles) {
-      const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
-      const uint32_t row = sr % P.n_rows;
-      const RowInfo ri = srow[row];
-      const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;
-      tensormap_fence_acquire(P.tmaps + sr);
-      mbar_arrive_expect_tx(&mbar[s], uint32_t(kBoxH) * ri.boxw * 2u);
-      tma_load_2d(tile_buf[s], P.tmaps + sr, -kPadHalo, (t0 - P.t_origin) - kReach, &mbar[s]);
-    }
+  // address and (clamped) length of a tile's digit list
+  auto tile_list = [&](uint32_t t, const uint32_t*& src) -> uint32_t {
+    const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
+    const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
+    const uint32_t cap = P.rows[row].cap;
+    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tt) * cap;
+    return min(P.counts[t], cap);
   };
-  if (tid == 0) {
-    for (int s = 0; s < kStages; ++s) fetch(s);
-  }
+  // stage digits [c0, c0+m) of a list in lbuf (one thread)
+  auto issue = [&](const uint32_t* src, uint32_t c0, uint32_t m) {
+    const uint32_t bytes = ((m + 3u) & ~3u) * 4u;              // bins are padded to a multiple of 4 digits
+    mbar_arrive_expect_tx(mbar, bytes);
+    tma_bulk_load(lbuf, src + c0, bytes, mbar);
+  };
+  // take the next tile in ticket order and start staging its list (one thread)
+  auto fetch = [&]() {
+    const uint32_t t = atomicAdd(&P.status->ticket, 1u);
+    uint32_t n = 0;
+    if (t < P.n_tiles) {
+      const uint32_t* src;
+      n = tile_list(t, src);
+      if (n) issue(src, 0, min(n, uint32_t(kDigCap)));
+    }
+    s_next[0] = t;
+    s_next[1] = n;
+  };
+  if (tid == kBuildThreads) fetch();
   __syncthreads();
 
-  uint32_t phase[kStages];
-#pragma unroll
-  for (int s = 0; s < kStages; ++s) phase[s] = 0;
-
-  for (int stage = 0;; stage = (stage + 1) % kStages) {
-    const uint32_t t = s_tile[stage];
+  uint32_t parity = 0;
+  for (;;) {
+    const uint32_t t = s_next[0], n = s_next[1];
     if (t >= P.n_tiles) break;
     const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
     const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
-    const RowInfo ri = srow[row];
+    const RowInfo ri = P.rows[row];
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
-    const uint32_t bmw = P.bm_words;
-    const uint16_t* tile = tile_buf[stage];
+    const uint32_t W = ri.W, wpr = W >> 1;
+    uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
+    uint32_t* bm = reinterpret_cast<uint32_t*>(mapraw + uint32_t(kBoxH) * W * 2u);   // W % 8 == 0: 16-byte aligned
+    const uint32_t* src = nullptr;
+    if (n > uint32_t(kDigCap)) tile_list(t, src);                        // only big tiles stage more than once
 
-    // clear the flag bitmap while the TMA load is in flight
-    for (uint32_t i = tid; i < kBoxH * bmw; i += kThreads) bm[i] = 0u;
-    __syncthreads();
-    mbar_wait(&mbar[stage], phase[stage]);
-    phase[stage] ^= 1u;
-
-    // ---------------- phase A (S2): D4 peak flags for tile rows 1 .. ncore+8 ----------------
-    // Each thread owns one 2-cell word column and walks a strip of rows, keeping the 3-cell
-    // horizontal maxima of the previous / current / next row in registers.
+    // ---- D2: zero the tile's charge map and flag bitmap (the list is landing meanwhile) ----
     {
-      const uint32_t wpr = ri.boxw >> 1;                 // 32-bit words per tile row
-      const uint32_t nw = ri.nwords;                     // active word columns (pads 0 .. npads-1)
-      const uint32_t nstrips = kThreads / nw;
-      const uint32_t strip = tid / nw, wc = tid - strip * nw;
-      const uint32_t R = ncore + 2 * (kReach - 1);       // rows 1..R get flags
-      const uint32_t rps = (R + nstrips - 1) / nstrips;
-      const uint32_t jb = 1 + strip * rps, je = min(jb + rps, R + 1);
-      if (strip < nstrips && jb < je) {
-        const uint32_t* t32 = reinterpret_cast<const uint32_t*>(tile) + (wc + kPadHalo / 2);
-        const uint32_t theta2 = P.theta | (P.theta << 16);
-        auto load3 = [&](uint32_t j, uint32_t& X, uint32_t& L, uint32_t& Rr) {
-          const uint32_t* p = t32 + j * wpr;
-          const uint32_t xl = p[-1], xr = p[1];          // halo words left and right are zero
-          X = p[0];
-          L = __byte_perm(xl, X, 0x5432);                // (pad-1, pad) for the low half, ...
-          Rr = __byte_perm(X, xr, 0x5432);               // (pad+1, pad+2)
-        };
-        uint32_t X, L, Rr, Xn, Ln, Rn;
-        load3(jb - 1, X, L, Rr);
-        uint32_t Hm = __vimax3_u16x2(L, X, Rr);          // 3-cell maxima of row j-1
-        load3(jb, X, L, Rr);
-        uint32_t H0 = __vimax3_u16x2(L, X, Rr);
-        for (uint32_t j = jb; j < je; ++j) {
-          load3(j + 1, Xn, Ln, Rn);
-          const uint32_t Hp = __vimax3_u16x2(Ln, Xn, Rn);
-          // D4: strictly greater than the 4 earlier neighbours (row j-1, and pad-1 in row j),
-          // >= the 4 later ones (pad+1 in row j, row j+1), and >= theta.  With integers
-          // Q > x  <=>  Q >= x+1.
-          const uint32_t be = __vmaxu2(L, Hm) + 0x00010001u;
-          const uint32_t bl = __vmaxu2(Rr, Hp);
-          const uint32_t bound = __vimax3_u16x2(be, bl, theta2);
-          const uint32_t pk = ((X | 0x80008000u) - bound) & 0x80008000u;   // bit15 of a half: Q >= bound
-          if (pk) {
-            const uint32_t bit0 = 2u * wc + 4u;                            // bitmap bit = pad + 4
-            if (pk & 0x00008000u) atomicOr(&bm[j * bmw + (bit0 >> 5)], 1u << (bit0 & 31u));
-            if (pk & 0x80000000u) atomicOr(&bm[j * bmw + ((bit0 + 1) >> 5)], 1u << ((bit0 + 1) & 31u));
-          }
-          Hm = H0; H0 = Hp; X = Xn; L = Ln; Rr = Rn;
-        }
+      const uint32_t nz = (uint32_t(kBoxH) * W * 2u + uint32_t(kBoxH) * bmw * 4u + 15u) >> 4;
+      uint4* z = reinterpret_cast<uint4*>(mapraw);
+      for (uint32_t i = tid; i < nz; i += kThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    __syncthreads();
+
+    // ---- S1: scatter the staged digits into the map ----
+    for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
+      const uint32_t m = min(n - c0, uint32_t(kDigCap));
+      if (c0) {
+        __syncthreads();
+        if (tid == kBuildThreads) issue(src, c0, m);
+      }
+      mbar_wait(mbar, parity);
+      parity ^= 1u;
+      for (uint32_t i = tid; i < m; i += kThreads) {
+        const uint32_t d = lbuf[i];
+        map[((d >> 8) & 0xFFu) * W + (d & 0xFFu) + kColOff] = uint16_t(d >> 16);
       }
     }
     __syncthreads();
 
-    // ---------------- phase B (S6): ordered count, tile prefix, global prefix ----------------
+    // ---- S2: D4 peak flags for map rows 1..136, digit-driven ----
+    {
+      const uint32_t* map32 = reinterpret_cast<const uint32_t*>(map);
+      for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
+        const uint32_t m = min(n - c0, uint32_t(kDigCap));
+        if (n > uint32_t(kDigCap)) {                                     // re-stage (the first pass overwrote lbuf)
+          __syncthreads();
+          if (tid == kBuildThreads) issue(src, c0, m);
+          mbar_wait(mbar, parity);
+          parity ^= 1u;
+        }
+        for (uint32_t i = tid; i < m; i += kThreads) {
+          const uint32_t d = lbuf[i];
+          const uint32_t q = d >> 16, tl = (d >> 8) & 0xFFu, pad = d & 0xFFu;
+          if (q >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q))
+            atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
+        }
+      }
+    }
+    __syncthreads();   // flags complete; lbuf is free
+
+    // ---- S6: ordered count of the core rows, block scan ----
     uint32_t cnt = 0;
     if (tid < ncore) {
       const uint32_t* r = bm + (kReach + tid) * bmw;
       for (uint32_t w = 0; w < bmw; ++w) cnt += __popc(r[w]);
     }
-    // block exclusive scan over kTileT (<= kThreads) row counts
     uint32_t incl = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t n = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= uint32_t(o)) incl += n;
+      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= uint32_t(o)) incl += v;
     }
     if (lane == 31) s_misc[1 + warp] = incl;
     __syncthreads();
@@ -503,69 +537,71 @@ __global__ void __launch_bounds__(kThreads, 2) k_cluster(const __grid_constant__
       total += v;
     }
     if (tid <= kTileT) rowoff[tid] = (tid < kTileT) ? (wbase + incl - cnt) : total;
-    if (warp == 0) {
+
+    if (warp == kBuildThreads / 32) {
+      // ---- dedicated warp: next tile's ticket + list staging, then the look-back of this tile ----
+      if (lane == 0) fetch();
       const uint32_t excl = lookback_exclusive(P.tile_state, t, P.epoch, total);
       if (lane == 0) {
         s_misc[0] = excl;
         if (t == P.n_tiles - 1) P.status->n_clusters = (unsigned long long)excl + total;
       }
-    }
-    __syncthreads();
-    const uint64_t gbase = s_misc[0];
-
-    // ---------------- phase C (S3..S5): clusters, kListCap peaks per pass ----------------
-    for (uint32_t done = 0; done < total;) {
-      // rows [r0, r1) whose peaks fit in the list: rowoff[r1] - done <= kListCap
-      // (a row holds at most 124 peaks, so every pass makes progress)
-      if (tid < ncore) {
-        const uint32_t ro = rowoff[tid], rn = ro + cnt;
-        if (ro >= done && rn - done <= kListCap && cnt) {
-          uint32_t k = ro - done;
-          const uint32_t* r = bm + (kReach + tid) * bmw;
-          for (uint32_t w = 0; w < bmw; ++w) {
-            uint32_t bits = r[w];
-            while (bits) {
-              const uint32_t b = __ffs(bits) - 1;
-              bits &= bits - 1;
-              plist[k++] = ((kReach + tid) << 16) | (w * 32 + b - 4);    // (tile row, pad)
+    } else {
+      // ---- S3..S5: clusters, kListCap peaks per pass, by warps 0..6 ----
+      for (uint32_t done = 0; done < total;) {
+        // rows whose peaks fit in the list: rowoff[r] + cnt - done <= kListCap
+        // (a row holds at most 124 peaks, so every pass makes progress)
+        if (tid < ncore) {
+          const uint32_t ro = rowoff[tid], rn = ro + cnt;
+          if (ro >= done && rn - done <= kListCap && cnt) {
+            uint32_t k = ro - done;
+            const uint32_t* r = bm + (kReach + tid) * bmw;
+            for (uint32_t w = 0; w < bmw; ++w) {
+              uint32_t bits = r[w];
+              while (bits) {
+                const uint32_t b = __ffs(bits) - 1;
+                bits &= bits - 1;
+                plist[k++] = ((kReach + tid) << 16) | (w * 32 + b - 4);    // (map row, pad)
+              }
             }
           }
         }
-      }
-      __syncthreads();
-      // number of peaks in this pass = largest rowoff[r] - done that is <= kListCap
-      uint32_t npass = min(total - done, uint32_t(kListCap));
-      if (total - done > kListCap) {
-        // find the last row boundary within the cap (all threads compute the same value)
-        uint32_t lo = 0, hi = ncore;               // rowoff is non-decreasing
-        while (hi - lo > 1) {
-          const uint32_t mid = (lo + hi) >> 1;
-          if (rowoff[mid] - done <= kListCap && rowoff[mid] >= done) lo = mid; else hi = mid;
+        bar_sync_named(1, kBuildThreads);
+        // number of peaks in this pass = largest rowoff[r] - done that is <= kListCap
+        uint32_t npass = min(total - done, uint32_t(kListCap));
+        if (total - done > kListCap) {
+          uint32_t lo = 0, hi = ncore;               // rowoff is non-decreasing
+          while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (rowoff[mid] - done <= kListCap && rowoff[mid] >= done) lo = mid; else hi = mid;
+          }
+          npass = (rowoff[hi] >= done && rowoff[hi] - done <= kListCap) ? rowoff[hi] - done : rowoff[lo] - done;
         }
-        // rowoff[hi] may still fit
-        npass = (rowoff[hi] >= done && rowoff[hi] - done <= kListCap) ? rowoff[hi] - done : rowoff[lo] - done;
-      }
-      for (uint32_t i = tid; i < npass; i += kThreads) {
-        const uint32_t e = plist[i];
-        const uint32_t j = e >> 16, pad = e & 0xFFFFu;
-        const uint64_t g = gbase + done + i;
-        if (g < P.out_capacity) {
-          ClusterRec rec;
-          build_cluster(tile, bm, ri.boxw, bmw, j, pad, sector, row, ri.npads, t0 + int32_t(j) - kReach,
-                        P.tf_time_bins, rec);
-          uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<ClusterRec*>(P.out) + g);
-          const uint4* s4 = reinterpret_cast<const uint4*>(&rec);
-          o[0] = s4[0];
-          o[1] = s4[1];
+        // first wave: one record per thread, built while the look-back is still running
+        ClusterRec rec;
+        const bool have = tid < npass;
+        if (have) {
+          const uint32_t e = plist[tid];
+          build_cluster(map, bm, W, bmw, e >> 16, e & 0xFFFFu, sector, row, ri.npads,
+                        t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, rec);
         }
+        if (done == 0) bar_sync_named(2, kThreads);  // look-back result (the dedicated warp arrives below)
+        const uint64_t gbase = uint64_t(s_misc[0]) + done;
+        if (have && gbase + tid < P.out_capacity) store_rec(P.out, gbase + tid, rec);
+        for (uint32_t i = tid + kBuildThreads; i < npass; i += kBuildThreads) {
+          if (gbase + i < P.out_capacity) {
+            const uint32_t e = plist[i];
+            build_cluster(map, bm, W, bmw, e >> 16, e & 0xFFFFu, sector, row, ri.npads,
+                          t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, rec);
+            store_rec(P.out, gbase + i, rec);
+          }
+        }
+        done += npass;
+        bar_sync_named(1, kBuildThreads);            // plist is rewritten by the next pass
       }
-      done += npass;
-      __syncthreads();
     }
-    __syncthreads();
-    // this stage's buffer is free: fetch the next tile into it
-    if (tid == 0) fetch(stage);
-    __syncthreads();
+    if (warp == kBuildThreads / 32 && total) bar_sync_named(2, kThreads);   // pairs with the "done == 0" barrier above
+    __syncthreads();   // map, bitmap and s_next are stable until here
   }
 }
 
