@@ -31,6 +31,7 @@ struct tpcclus_ctx {
   uint32_t max_tiles = 0;
   uint32_t map_bytes_max = 0, bm_words = 0, smem_bytes = 0;
   int tile_grid = 0;              // persistent grid of k_tile
+  bool bin_aggregated = false;    // k_bin (CTA-aggregated) usable for this geometry, else k_bin_direct
   int n_sm = 0;
   uint32_t epoch = 0;
   uint64_t launches = 0;
@@ -215,6 +216,14 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tile, kThreads, c->smem_bytes) != cudaSuccess || occ < 1)
     return fail(TPCCLUS_ERR_CUDA);
   c->tile_grid = occ * c->n_sm;
+  {
+    const uint32_t nb_max = g->n_rows * c->tiles_per_row_max;
+    c->bin_aggregated = nb_max <= kBinMaxNb && bin_smem_bytes(nb_max) <= uint32_t(prop.sharedMemPerBlockOptin) &&
+                        !std::getenv("TPCCLUS_BIN_DIRECT");
+    if (c->bin_aggregated &&
+        cudaFuncSetAttribute(k_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bin_smem_bytes(nb_max))) != cudaSuccess)
+      return fail(TPCCLUS_ERR_CUDA);
+  }
 
   if (g->options & TPCCLUS_OPT_HOST_STAGING) {
     for (int i = 0; i < 2; ++i) {
@@ -282,10 +291,31 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     bp.tiles_per_row = tiles_per_row;
     bp.tiles_per_row_max = c->tiles_per_row_max;
     std::memcpy(bp.off, h_off, (g.n_sectors + 1) * sizeof(uint64_t));
-    const uint64_t pairs = (n + 1) / 2;
-    const uint32_t blocks = uint32_t(std::min<uint64_t>((pairs + 255) / 256, uint64_t(c->n_sm) * 16));
-    k_bin<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), bp, c->d_rows, c->d_lists,
-                                                c->d_counts, c->d_status);
+    bp.nb = g.n_rows * tiles_per_row;
+    if (c->bin_aggregated && bp.nb <= kBinMaxNb) {
+      // CTA-aggregated binning: chunks of kBinChunk digits, one sector per chunk
+      bp.head = (reinterpret_cast<uintptr_t>(d_digits) & 8u) ? 1u : 0u;
+      bp.base16 = reinterpret_cast<const uint4*>(reinterpret_cast<uintptr_t>(d_digits) - 8u * bp.head);
+      bp.pair_lo = bp.head;
+      bp.pair_hi = (n + bp.head) >> 1;
+      uint64_t cps = 0;
+      for (uint32_t s = 0; s < g.n_sectors; ++s) {
+        if (h_off[s + 1] <= h_off[s]) continue;
+        const uint64_t p0 = std::max<uint64_t>((h_off[s] + bp.head) >> 1, bp.pair_lo);
+        const uint64_t p1 = std::min<uint64_t>((h_off[s + 1] + bp.head + 1) >> 1, bp.pair_hi);
+        if (p1 > p0) cps = std::max<uint64_t>(cps, (p1 - p0 + kBinChunk / 2 - 1) / (kBinChunk / 2));
+      }
+      bp.chunks_per_sector = uint32_t(cps);
+      bp.pad_ = 0;
+      const uint64_t total = uint64_t(g.n_sectors) * cps;
+      const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(total, 1), uint64_t(c->n_sm)));
+      k_bin<<<blocks, kBinThreads, bin_smem_bytes(bp.nb), st>>>(bp, c->d_rows, c->d_lists, c->d_counts, c->d_status);
+    } else {
+      const uint64_t pairs = (n + 1) / 2;
+      const uint32_t blocks = uint32_t(std::min<uint64_t>((pairs + 255) / 256, uint64_t(c->n_sm) * 16));
+      k_bin_direct<<<std::max(blocks, 1u), 256, 0, st>>>(reinterpret_cast<const uint2*>(d_digits), bp, c->d_rows,
+                                                         c->d_lists, c->d_counts, c->d_status);
+    }
     c->launches++;
     debug_check(st, "k_bin");
   }

@@ -59,6 +59,13 @@ struct BinParams {
   uint32_t n_sectors, n_rows;
   uint32_t tiles_per_row;              // tiles of this run
   uint32_t tiles_per_row_max;          // bins laid out per (sector,row)
+  // k_bin (CTA-aggregated binning) only:
+  const uint4* base16;                 // digit buffer aligned down to 16 bytes; digit i is 8-byte slot i + head
+  uint32_t head;                       // 1 if the buffer starts in the upper half of a 16-byte pair
+  uint32_t nb;                         // bins per sector of this run = n_rows * tiles_per_row
+  uint32_t chunks_per_sector;          // max over sectors of ceil(pairs / (kBinChunk/2))
+  uint32_t pad_;
+  uint64_t pair_lo, pair_hi;           // pairs with both slots inside the buffer: [pair_lo, pair_hi)
   uint64_t off[kMaxSectors + 1];       // sector offsets (copied from the host array)
 };
 
@@ -164,6 +171,12 @@ __global__ void __launch_bounds__(256) k_init(uint32_t* __restrict__ counts, uin
 // A bin has one slot per map cell, so it cannot overflow while D2's precondition (at most one
 // digit per cell) holds; slots past the capacity are discarded (memory-safe for duplicates).
 // ----------------------------------------------------------------------------------------
+// packed list entry: pad (8 bits) | tl << 8 (row of the tile window, 9 bits) | q16 << 17 (14 bits)
+__device__ __forceinline__ uint32_t pack_digit(uint32_t pad, uint32_t tl, uint32_t q) { return pad | (tl << 8) | (q << 17); }
+__device__ __forceinline__ uint32_t dig_pad(uint32_t d) { return d & 0xFFu; }
+__device__ __forceinline__ uint32_t dig_tl(uint32_t d) { return (d >> 8) & 0x1FFu; }
+__device__ __forceinline__ uint32_t dig_q(uint32_t d) { return d >> 17; }
+
 __device__ __forceinline__ uint32_t quantise_q16(float charge) {
   // D1: q16 = clamp(rint(charge*16), 0, 16368); rint = round-half-even (cvt.rni); NaN -> 0
   const float x = rintf(charge * 16.0f);
@@ -191,12 +204,12 @@ __device__ __forceinline__ bool bin_one(uint32_t w0, uint32_t w1, uint64_t idx, 
   for (int32_t tt = tt_lo; tt <= tt_hi; ++tt) {
     const uint32_t tl = uint32_t(u - tt * kTileT + kReach);      // 0..137
     const uint32_t slot = atomicAdd(&counts[sr * P.tiles_per_row + uint32_t(tt)], 1u);
-    if (slot < ri.cap) lists[base + uint64_t(tt) * ri.cap + slot] = pad | (tl << 8) | (q << 16);
+    if (slot < ri.cap) lists[base + uint64_t(tt) * ri.cap + slot] = pack_digit(pad, tl, q);
   }
   return true;
 }
 
-__global__ void __launch_bounds__(256) k_bin(const uint2* __restrict__ digits, const __grid_constant__ BinParams P,
+__global__ void __launch_bounds__(256) k_bin_direct(const uint2* __restrict__ digits, const __grid_constant__ BinParams P,
                                              const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
                                              uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
   __shared__ RowInfo srow[256];
@@ -237,6 +250,188 @@ __global__ void __launch_bounds__(256) k_bin(const uint2* __restrict__ digits, c
   // warp-aggregated count of dropped digits
   dropped = __reduce_add_sync(0xffffffffu, dropped);
   if ((threadIdx.x & 31) == 0 && dropped) atomicAdd(&status->n_dropped, (unsigned long long)dropped);
+}
+
+// ----------------------------------------------------------------------------------------
+// S1 (first half), CTA-aggregated: the production binning kernel.
+//
+// Why: with one global atomic per list entry (k_bin_direct) the kernel is bound by the L2
+// atomic units — all CTAs hammer the ~5000 contiguous counters of the sector being read
+// (profiles/r1b_bin_tile_ncu.md, 5.7 ms for 3.4e8 atomics).  Here a CTA takes a CHUNK of
+// 16384 digits of ONE sector, staged in shared memory by TMA bulk copies that land while the
+// previous chunk is still being written out, ranks every digit inside its bin with a
+// shared-memory atomic, reserves the chunk's slots with ONE global atomic per non-empty bin,
+// and then stores the packed digits.  Chunks are dealt round-robin over the sectors so that
+// concurrently running CTAs reserve in different sectors' counters.
+// ----------------------------------------------------------------------------------------
+constexpr int      kBinThreads  = 1024;
+constexpr int      kBinPer      = 16;                       // digits per thread per chunk
+constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 16384 digits = 128 KB of input
+constexpr uint32_t kBinMaxNb    = 16384;                    // bins per sector the histogram can hold
+constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room for this chunk (duplicates only)
+constexpr int      kTileShift   = 7;
+static_assert((1 << kTileShift) == kTileT, "tile size is a power of two");
+
+__host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
+  return uint32_t(kBinChunk) * 8u + ((nb + 3u) & ~3u) * 4u + 3u * 256u * 4u + 64u;
+}
+
+__global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ BinParams P,
+                                                        const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
+                                                        uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  const uint4* stage = reinterpret_cast<const uint4*>(sp);   sp += uint32_t(kBinChunk) * 8u;   // TMA destination
+  uint32_t* hist = reinterpret_cast<uint32_t*>(sp);           sp += ((P.nb + 3u) & ~3u) * 4u;
+  uint32_t* r_npads = reinterpret_cast<uint32_t*>(sp);        sp += 256 * 4;
+  uint32_t* r_off = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
+  uint32_t* r_cap = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);           sp += 16;
+  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);         sp += 16;
+
+  const uint32_t tid = threadIdx.x;
+  for (uint32_t i = tid; i < 256u; i += kBinThreads) {
+    const bool in = i < P.n_rows;
+    r_npads[i] = in ? rows[i].npads : 0u;
+    r_off[i] = in ? rows[i].list_off : 0u;
+    r_cap[i] = in ? rows[i].cap : 0u;
+  }
+  if (tid == 0) {
+    mbar_init(mbar, 1);
+    fence_mbar_init();
+  }
+  uint32_t dropped = 0;
+  // the (at most two) digits that do not sit in a full 16-byte pair: direct path, one thread
+  if (blockIdx.x == 0 && tid == 32) {
+    const uint2* dg = reinterpret_cast<const uint2*>(P.base16) + P.head;
+    uint64_t edge[2];
+    int ne = 0;
+    if (P.head && P.n > 0) edge[ne++] = 0;
+    if (((P.n + P.head) & 1ull) && P.n > 0 && !(P.head && P.n == 1)) edge[ne++] = P.n - 1;
+    for (int k = 0; k < ne; ++k) {
+      uint32_t s0 = 0;
+      const uint2 v = dg[edge[k]];
+      dropped += bin_one(v.x, v.y, edge[k], s0, P, rows, lists, counts) ? 0u : 1u;
+    }
+  }
+
+  constexpr uint32_t kPairs = kBinChunk / 2;
+  const uint32_t total = P.n_sectors * P.chunks_per_sector;
+  // pair range of chunk k (sector k % n_sectors, chunk k / n_sectors of it); false if empty
+  auto chunk = [&](uint32_t k, uint32_t& s, uint64_t& pa, uint32_t& np) -> bool {
+    s = k % P.n_sectors;
+    const uint32_t ci = k / P.n_sectors;
+    const uint64_t p0 = max((P.off[s] + P.head) >> 1, P.pair_lo);
+    const uint64_t p1 = min((P.off[s + 1] + P.head + 1) >> 1, P.pair_hi);
+    pa = p0 + uint64_t(ci) * kPairs;
+    if (P.off[s + 1] <= P.off[s] || pa >= p1) return false;
+    np = uint32_t(min(uint64_t(kPairs), p1 - pa));
+    return true;
+  };
+  // one thread: find the next non-empty chunk at or after k (stride gridDim.x), start its TMA
+  auto fetch = [&](uint32_t k) {
+    uint32_t s = 0, np = 0;
+    uint64_t pa = 0;
+    while (k < total && !chunk(k, s, pa, np)) k += gridDim.x;
+    if (k < total) {
+      mbar_arrive_expect_tx(mbar, np * 16u);
+      for (uint32_t o = 0; o < np; o += 2048u)            // <= 32 KB per bulk copy
+        tma_bulk_load(const_cast<uint4*>(stage) + o, P.base16 + pa + o, min(2048u, np - o) * 16u, mbar);
+    }
+    s_next[0] = k;
+  };
+  __syncthreads();
+  if (tid == 0) fetch(blockIdx.x);
+  __syncthreads();
+
+  uint32_t parity = 0;
+  for (;;) {
+    const uint32_t k = s_next[0];
+    if (k >= total) break;
+    uint32_t s, np;
+    uint64_t pa;
+    chunk(k, s, pa, np);
+    const uint64_t d_lo = P.off[s], d_hi = P.off[s + 1];     // digits of this sector
+    for (uint32_t i = tid; i < P.nb; i += kBinThreads) hist[i] = 0u;
+    __syncthreads();
+    mbar_wait(mbar, parity);
+    parity ^= 1u;
+
+    // ---- phase 1: quantise (D1), validate, rank inside the bin (shared-memory atomics) ----
+    uint32_t pk[kBinPer];            // packed digit for its first tile
+    uint32_t br[kBinPer];            // bin | rank << 14 | second-tile << 29 | valid << 30
+    uint32_t r2[kBinPer / 2];        // ranks in the second tile, two per word
+#pragma unroll
+    for (int j = 0; j < kBinPer / 2; ++j) {
+      const uint32_t pi = uint32_t(j) * kBinThreads + tid;
+      uint4 v = make_uint4(0u, 0u, 0u, 0u);
+      if (pi < np) v = stage[pi];
+      const uint64_t i0 = 2ull * (pa + pi) - P.head;         // digit index of the low slot
+      r2[j] = 0u;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t w0 = h ? v.z : v.x, w1 = h ? v.w : v.y;
+        const uint64_t idx = i0 + uint64_t(h);
+        uint32_t pkv = 0u, brv = 0u;
+        if (pi < np && idx >= d_lo && idx < d_hi) {
+          const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
+          const int32_t time = int32_t(w0 >> 16);
+          const uint32_t q = quantise_q16(__uint_as_float(w1));
+          if (q == 0u || time < P.t_lo || time >= P.t_hi || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
+            ++dropped;
+          } else {
+            const int32_t u = time - P.t_core_begin;
+            const int32_t tlo = max((u - kReach) >> kTileShift, 0);
+            const int32_t thi = min((u + kReach) >> kTileShift, int32_t(P.tiles_per_row) - 1);
+            if (tlo <= thi) {
+              const uint32_t bin = row * P.tiles_per_row + uint32_t(tlo);
+              pkv = pack_digit(pad, uint32_t(u - (tlo << kTileShift) + kReach), q);
+              brv = bin | (atomicAdd(&hist[bin], 1u) << 14) | (1u << 30);
+              if (thi != tlo) {
+                brv |= 1u << 29;
+                r2[j] |= atomicAdd(&hist[bin + 1u], 1u) << (16 * h);
+              }
+            }
+          }
+        }
+        pk[2 * j + h] = pkv;
+        br[2 * j + h] = brv;
+      }
+    }
+    __syncthreads();                  // stage is consumed, hist is complete
+
+    // ---- phase 2: next chunk's TMA; one global reservation per non-empty bin ----
+    if (tid == 0) fetch(k + gridDim.x);
+    for (uint32_t b = tid; b < P.nb; b += kBinThreads) {
+      const uint32_t c = hist[b];
+      if (c) {
+        const uint32_t row = b / P.tiles_per_row, tt = b - row * P.tiles_per_row;
+        const uint32_t cap = r_cap[row];
+        const uint32_t base = atomicAdd(&counts[s * P.nb + b], c);
+        hist[b] = (base + c <= cap) ? r_off[row] + tt * cap + base : kBinFull;
+      }
+    }
+    __syncthreads();
+
+    // ---- phase 3: store the packed digits at base + rank ----
+    uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
+#pragma unroll
+    for (int i = 0; i < kBinPer; ++i) {
+      const uint32_t b = br[i];
+      if (b & (1u << 30)) {
+        const uint32_t bin = b & 0x3FFFu;
+        const uint32_t e = hist[bin];
+        if (e != kBinFull) seclist[e + ((b >> 14) & 0x7FFFu)] = pk[i];
+        if (b & (1u << 29)) {
+          const uint32_t e2 = hist[bin + 1u];
+          if (e2 != kBinFull) seclist[e2 + ((r2[i >> 1] >> (16 * (i & 1))) & 0xFFFFu)] = pk[i] - (uint32_t(kTileT) << 8);
+        }
+      }
+    }
+    __syncthreads();                  // hist and s_next are stable until here
+  }
+  dropped = __reduce_add_sync(0xffffffffu, dropped);
+  if ((tid & 31u) == 0u && dropped) atomicAdd(&status->n_dropped, (unsigned long long)dropped);
 }
 
 // ----------------------------------------------------------------------------------------
@@ -489,7 +684,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       parity ^= 1u;
       for (uint32_t i = tid; i < m; i += kThreads) {
         const uint32_t d = lbuf[i];
-        map[((d >> 8) & 0xFFu) * W + (d & 0xFFu) + kColOff] = uint16_t(d >> 16);
+        map[dig_tl(d) * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));
       }
     }
     __syncthreads();
@@ -507,7 +702,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
         }
         for (uint32_t i = tid; i < m; i += kThreads) {
           const uint32_t d = lbuf[i];
-          const uint32_t q = d >> 16, tl = (d >> 8) & 0xFFu, pad = d & 0xFFu;
+          const uint32_t q = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
           if (q >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q))
             atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
         }
