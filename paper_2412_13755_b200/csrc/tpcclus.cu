@@ -47,12 +47,12 @@ struct tpcclus_ctx {
   struct Pending { uint64_t n, cap; };
   Pending pending[kRing];
   cudaEvent_t ev_done[kRing] = {};
-  cudaEvent_t ev_prof[kRing][4] = {};   // around k_init / k_bin / k_tile when profiling
+  cudaEvent_t ev_prof[kRing][TPCCLUS_N_KERNELS + 1] = {};   // around k_init / k_bin / k_tile / k_finish when profiling
   bool slot_profiled[kRing] = {};
   uint64_t head = 0, tail = 0;          // runs reported / runs enqueued
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
-  double prof_ms[3] = {0, 0, 0};
+  double prof_ms[TPCCLUS_N_KERNELS] = {};
   uint64_t prof_runs = 0;
   int sticky = TPCCLUS_OK;
   int sticky_cuda = 0;
@@ -124,7 +124,7 @@ void tpcclus_destroy(tpcclus_ctx* c) {
   if (c->tail != c->head) cudaStreamSynchronize(c->last_stream);
   for (int i = 0; i < kRing; ++i) {
     if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
-    for (int k = 0; k < 4; ++k) if (c->ev_prof[i][k]) cudaEventDestroy(c->ev_prof[i][k]);
+    for (int k = 0; k <= TPCCLUS_N_KERNELS; ++k) if (c->ev_prof[i][k]) cudaEventDestroy(c->ev_prof[i][k]);
   }
   cudaFree(c->d_lists); cudaFree(c->d_counts); cudaFree(c->d_rows); cudaFree(c->d_tile_state); cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
@@ -190,7 +190,8 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * c->tiles_per_row_max;
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
-  c->smem_bytes = kDigCap * 4 + c->map_bytes_max + 16 + 16 + 16 * 4 + kListCap * 4 + (kTileT + 4) * 4 + 128;
+  c->smem_bytes = kDigCap * 4 + c->map_bytes_max + 2 * kListCap * 32 + 16 + 16 + 16 * 4 + 2 * 4 * 4 + kListCap * 4 +
+                  (kTileT + 4) * 4 + kNbrTabWords * 4 + 12 * 4 + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;
@@ -202,7 +203,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (cudaMallocHost(reinterpret_cast<void**>(&c->h_status), kRing * sizeof(DevStatus)) != cudaSuccess) return fail(TPCCLUS_ERR_NOMEM);
   for (int i = 0; i < kRing; ++i) {
     if (cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k <= TPCCLUS_N_KERNELS; ++k)
       if (cudaEventCreate(&c->ev_prof[i][k]) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
   }
   if (cudaMemcpy(c->d_rows, c->rows.data(), g->n_rows * sizeof(RowInfo), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -349,6 +350,15 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     debug_check(st, "k_tile");
   }
   if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][3], st));
+  // S5 finish (D8): exact integer moments -> float32 fields, in place
+  if (cap) {
+    const uint64_t want = (std::min<uint64_t>(cap, g.max_clusters ? g.max_clusters : cap) + 255) / 256;
+    const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(want, 1), uint64_t(c->n_sm) * 8));
+    k_finish<<<blocks, 256, 0, st>>>(d_out, cap, c->d_status);
+    c->launches++;
+    debug_check(st, "k_finish");
+  }
+  if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][4], st));
   CK(c, cudaGetLastError());
   CK(c, cudaMemcpyAsync(&c->h_status[slot], c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));
   CK(c, cudaEventRecord(c->ev_done[slot], st));
@@ -374,7 +384,7 @@ int tpcclus_result(tpcclus_ctx* c, tpcclus_run_stats* stats) {
     return TPCCLUS_ERR_CUDA;
   }
   if (c->slot_profiled[slot]) {
-    for (int k = 0; k < 3; ++k) {
+    for (int k = 0; k < TPCCLUS_N_KERNELS; ++k) {
       float ms = 0.f;
       if (cudaEventElapsedTime(&ms, c->ev_prof[slot][k], c->ev_prof[slot][k + 1]) == cudaSuccess) c->prof_ms[k] += ms;
     }
@@ -392,13 +402,13 @@ int tpcclus_result(tpcclus_ctx* c, tpcclus_run_stats* stats) {
 int tpcclus_set_profiling(tpcclus_ctx* c, int on) {
   if (!c) return TPCCLUS_ERR_INVALID;
   c->profiling = on != 0;
-  if (on) { c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0; c->prof_runs = 0; }
+  if (on) { for (double& m : c->prof_ms) m = 0; c->prof_runs = 0; }
   return TPCCLUS_OK;
 }
 
-int tpcclus_get_profile(const tpcclus_ctx* c, double kernel_ms[3], uint64_t* n_runs) {
+int tpcclus_get_profile(const tpcclus_ctx* c, double kernel_ms[TPCCLUS_N_KERNELS], uint64_t* n_runs) {
   if (!c || !kernel_ms || !n_runs) return TPCCLUS_ERR_INVALID;
-  for (int k = 0; k < 3; ++k) kernel_ms[k] = c->prof_ms[k];
+  for (int k = 0; k < TPCCLUS_N_KERNELS; ++k) kernel_ms[k] = c->prof_ms[k];
   *n_runs = c->prof_runs;
   return TPCCLUS_OK;
 }

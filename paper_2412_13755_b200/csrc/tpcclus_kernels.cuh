@@ -26,12 +26,12 @@
 namespace tpcclus {
 
 constexpr int      kThreads      = 256;   // CTA size of k_tile
-constexpr int      kBuildThreads = 224;   // warps 0..6 build clusters; warp 7 prefetches and looks back
+constexpr int      kWorkThreads  = 224;   // warps 0..6 run S1..S5 on the tiles; warp 7 commits (look-back + copy-out)
 constexpr int      kTileT        = 128;   // core time bins per tile
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
-constexpr int      kListCap      = 1024;  // peaks processed per pass inside one tile
+constexpr int      kListCap      = 160;   // peaks per hand-over item (capacity of one staging buffer)
 constexpr int      kDigCap       = 4096;  // digits staged per TMA bulk copy (16 KB)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
@@ -460,7 +460,7 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
     if (lane == 0) st_release_u64(state, pack_state(epoch, kStPrefix, aggregate));
     return 0;
   }
-  if (lane == 0) st_release_u64(state + tile, pack_state(epoch, kStAgg, aggregate));
+  // the tile's own count (kStAgg) was published by its workers right after the count phase
   uint32_t sum = 0;
   int64_t look = int64_t(tile) - 1;
   while (true) {
@@ -486,101 +486,154 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
   return sum;
 }
 
-__device__ __constant__ uint16_t kShareWeight[10] = {0, 2520, 1260, 840, 630, 504, 420, 360, 315, 280};  // D6: L/S
+// ----------------------------------------------------------------------------------------
+// S3..S5, four lanes per peak.
+//
+// The 24 cells around a peak P split into four rotation classes of six: lane `sub` (0..3) owns
+// the images under the quarter turn R_sub of the base cells
+//     I0 = (1,0)  I1 = (1,1)                      inner ring (always members when charged, D5)
+//     O0 = (2,-1) O1 = (2,0) O2 = (2,1) O3 = (2,2) outer ring (monotone descent, D5)
+// written (a,b) = (pad, time) offsets in the lane's own frame; R_s(a,b) = (a cs - b sn, a sn + b cs)
+// with (cs,sn) = (1,0),(0,1),(-1,0),(0,-1).  The inner cells 8-adjacent to O0..O3 are
+// (1,-1),(1,0),(1,1) of the same frame, so a lane reads 7 charges.  Moments are summed in the
+// lane frame with constant coefficients and rotated once.  D6's S(c) comes from the OTHER peaks
+// of the 9x9 flag window: each one adds a table entry (one nibble per owned cell it is within
+// distance 2 of, plus an "is this outer cell" bit).  The four partial sums are combined with two
+// xor-shuffles; the record is written as exact integers (RawRec) and finished by k_finish.
+// ----------------------------------------------------------------------------------------
+constexpr int kNbrTabWords = 4 * 81;
+constexpr uint32_t kShareL = 2520u;                      // D6: lcm(1..9)
 
-// One thread builds one cluster (S3..S5).  map: smem charges [kBoxH][W], column = pad + kColOff;
-// bm: smem flag bitmap [kBoxH][bmw], bit (pad+4) of row j set iff the cell is a peak (D4).
-__device__ __forceinline__ void build_cluster(const uint16_t* __restrict__ map, const uint32_t* __restrict__ bm,
-                                              uint32_t W, uint32_t bmw, uint32_t j, uint32_t pad,
-                                              uint32_t sector, uint32_t row, uint32_t npads, int32_t tglob,
-                                              uint32_t tf_time_bins, ClusterRec& rec) {
-  // 5x5 charges around the peak: map column of pad p is p + kColOff
-  uint32_t q[5][5];
-  const uint16_t* c0 = map + (j - 2) * W + (pad + kColOff - 2);
-#pragma unroll
-  for (int dt = 0; dt < 5; ++dt)
-#pragma unroll
-    for (int dp = 0; dp < 5; ++dp) q[dt][dp] = c0[dt * W + dp];
-
-  // 9x9 peak-flag window: F[k] bit i  <->  row j-4+k, pad  p-4+i  (bitmap bit = pad + 4)
-  uint32_t F[9];
-  uint32_t others = 0;
-  {
-    const uint32_t sh = pad & 31u, wi = pad >> 5;
-#pragma unroll
-    for (int k = 0; k < 9; ++k) {
-      const uint32_t* rowp = bm + (j - 4 + k) * bmw + wi;
-      F[k] = __funnelshift_r(rowp[0], rowp[1], sh) & 0x1FFu;
-      others |= (k == 4) ? (F[k] & ~0x10u) : F[k];
-    }
+// entry for lane frame s and another peak at window row k (time j-4+k), column i (pad p-4+i)
+__device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
+  const int s = int(idx / 81u), r = int(idx % 81u);
+  const int u = r % 9 - 4, v = r / 9 - 4;               // (pad, time) offset of the other peak
+  int up, vp;                                           // the same offset in the lane frame: R_s^-1 (u,v)
+  if (s == 0)      { up = u;  vp = v; }
+  else if (s == 1) { up = v;  vp = -u; }
+  else if (s == 2) { up = -u; vp = -v; }
+  else             { up = -v; vp = u; }
+  const int ca[6] = {1, 1, 2, 2, 2, 2}, cb[6] = {0, 1, -1, 0, 1, 2};
+  uint32_t e = 0;
+  for (int c = 0; c < 6; ++c) {
+    const int da = ca[c] - up, db = cb[c] - vp;
+    if (da >= -2 && da <= 2 && db >= -2 && db <= 2) e += 1u << (4 * c);
+    if (c >= 2 && da == 0 && db == 0) e |= 1u << (24 + c - 2);
   }
-
-  const uint32_t qP = q[2][2];
-  uint32_t W_ = qP * 2520u, Mpp = 0, Mtt = 0, ncells = 1, flags = 0;
-  int32_t Mp = 0, Mt = 0;
-  if (qP == kQClamp) flags |= 4u;
-#pragma unroll
-  for (int dt = -2; dt <= 2; ++dt)
-#pragma unroll
-    for (int dp = -2; dp <= 2; ++dp) {
-      if (dp == 0 && dt == 0) continue;
-      const uint32_t qc = q[dt + 2][dp + 2];
-      bool member = qc != 0u;                                  // D5: a member has charge
-      const bool outer = (dp == -2 || dp == 2 || dt == -2 || dt == 2);
-      if (outer) {
-        // D5: a peak is never a member; an inner-ring cell cannot be a peak (adjacent to P)
-        member = member && !((F[dt + 4] >> (dp + 4)) & 1u);
-        // D5 outer ring: some inner-ring cell 8-adjacent to c with Q(i) >= Q(c)
-        bool desc = false;
-#pragma unroll
-        for (int it = -1; it <= 1; ++it)
-#pragma unroll
-          for (int ip = -1; ip <= 1; ++ip) {
-            if (ip == 0 && it == 0) continue;
-            if (ip - dp > 1 || dp - ip > 1 || it - dt > 1 || dt - it > 1) continue;
-            desc = desc || (q[it + 2][ip + 2] >= qc);
-          }
-        member = member && desc;
-      }
-      if (member) {
-        uint32_t S = 1;
-        if (others) {                                          // D6: peaks within distance 2 of c
-          S = 0;
-#pragma unroll
-          for (int jt = -2; jt <= 2; ++jt) S += __popc((F[dt + jt + 4] >> (dp + 2)) & 0x1Fu);
-        }
-        const uint32_t w = qc * uint32_t(kShareWeight[S]);     // D6 weight in 1/(16*2520) ADC
-        W_ += w;                                               // D7 moments, exact integers
-        Mp += int32_t(w) * dp;
-        Mt += int32_t(w) * dt;
-        Mpp += w * uint32_t(dp * dp);
-        Mtt += w * uint32_t(dt * dt);
-        ++ncells;
-        if (S >= 2) flags |= 8u;
-        if (qc == kQClamp) flags |= 4u;
-      }
-    }
-  if (pad < 2u || pad + 2u >= npads) flags |= 1u;              // D8 EDGE_PAD
-  if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
-  // D8: evaluated in double from the exact integers, rounded once to float32
-  const double Wd = double(W_);
-  const long long Np = (long long)Mpp * (long long)W_ - (long long)Mp * (long long)Mp;
-  const long long Nt = (long long)Mtt * (long long)W_ - (long long)Mt * (long long)Mt;
-  rec.w0 = sector | (row << 8) | (pad << 16) | (flags << 24);
-  rec.time = uint32_t(tglob);
-  rec.w2 = qP | (ncells << 16);
-  rec.qtot = float(Wd / 40320.0);
-  rec.dpad = float(double(Mp) / Wd);
-  rec.dtime = float(double(Mt) / Wd);
-  rec.sigma_pad = float(sqrt(double(Np)) / Wd);
-  rec.sigma_time = float(sqrt(double(Nt)) / Wd);
+  return e;
 }
 
-__device__ __forceinline__ void store_rec(void* out, uint64_t g, const ClusterRec& rec) {
-  uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<ClusterRec*>(out) + g);
-  const uint4* s4 = reinterpret_cast<const uint4*>(&rec);
-  o[0] = s4[0];
-  o[1] = s4[1];
+struct __align__(16) RawRec {       // what k_tile writes: D7's exact integers; k_finish turns it into ClusterRec in place
+  uint32_t w0, time, w2;            // as in ClusterRec
+  uint32_t W;                       // sum of weights, units of 1/(16*2520) ADC
+  int32_t Mp, Mt;                   // sum w dp, sum w dt
+  uint32_t Mpp, Mtt;                // sum w dp^2, sum w dt^2
+};
+static_assert(sizeof(RawRec) == 32, "raw record is 32 bytes");
+
+// All 32 lanes call this; lanes 4g..4g+3 work on the same peak (j = map row, pad).  Returns the
+// two 16-byte halves of the RawRec in every lane of the group.
+__device__ __forceinline__ void build_cluster4(const uint16_t* __restrict__ map, const uint32_t* __restrict__ bm,
+                                               const uint32_t* __restrict__ nbr_tab, const uint32_t* __restrict__ wtab,
+                                               uint32_t W, uint32_t bmw, uint32_t j, uint32_t pad, uint32_t sub,
+                                               int32_t cs, int32_t sn, uint32_t sector, uint32_t row, uint32_t npads,
+                                               int32_t tglob, uint32_t tf_time_bins, uint4& lo, uint4& hi) {
+  const uint16_t* c = map + j * W + (pad + kColOff);
+  const int32_t X = sn * int32_t(W) + cs, Y = cs * int32_t(W) - sn;     // steps of (a,b) in map cells
+  const uint32_t qP = c[0];
+  const uint32_t qIm = c[X - Y], qI0 = c[X], qI1 = c[X + Y];
+  const uint32_t qO0 = c[2 * X - Y], qO1 = c[2 * X], qO2 = c[2 * X + Y], qO3 = c[2 * X + 2 * Y];
+
+  // 9x9 flag window packed three rows per word: bit 9*(k%3)+i of G[k/3] <-> row j-4+k, pad p-4+i
+  uint32_t G0 = 0, G1 = 0, G2 = 0;
+  {
+    const uint32_t sh = pad & 31u;
+    const uint32_t* rowp = bm + (j - 4u) * bmw + (pad >> 5);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+      const uint32_t f = __funnelshift_r(rowp[k * bmw], rowp[k * bmw + 1], sh) & 0x1FFu;
+      if (k < 3) G0 |= f << (9 * k);
+      else if (k < 6) G1 |= f << (9 * (k - 3));
+      else G2 |= f << (9 * (k - 6));
+    }
+    G1 &= ~(1u << 13);                                                  // P itself (row 4, column 4)
+  }
+  uint32_t acc = 0;                                                     // nibble c: other peaks within distance 2 of cell c
+  {
+    const uint32_t* t = nbr_tab + sub * 81u;
+    while (G0) { const uint32_t b = __ffs(G0) - 1; G0 &= G0 - 1; acc += t[b]; }
+    while (G1) { const uint32_t b = __ffs(G1) - 1; G1 &= G1 - 1; acc += t[27 + b]; }
+    while (G2) { const uint32_t b = __ffs(G2) - 1; G2 &= G2 - 1; acc += t[54 + b]; }
+  }
+  // D5 membership
+  const bool mI0 = qI0 != 0u, mI1 = qI1 != 0u;
+  const bool mO0 = qO0 != 0u && !((acc >> 24) & 1u) && (qIm >= qO0 || qI0 >= qO0);
+  const bool mO1 = qO1 != 0u && !((acc >> 25) & 1u) && (qIm >= qO1 || qI0 >= qO1 || qI1 >= qO1);
+  const bool mO2 = qO2 != 0u && !((acc >> 26) & 1u) && (qI0 >= qO2 || qI1 >= qO2);
+  const bool mO3 = qO3 != 0u && !((acc >> 27) & 1u) && (qI1 >= qO3);
+  // D6 weights w = Q * L / S, S = 1 + other peaks within distance 2
+  uint32_t meta = 0;                                                    // ncells | n_saturated << 8 | n_split << 16
+  auto weight = [&](bool m, uint32_t q, uint32_t nib) -> uint32_t {
+    const uint32_t S = (acc >> (4 * nib)) & 15u;                        // S - 1
+    if (m) meta += 1u + (q == kQClamp ? 0x100u : 0u) + (S ? 0x10000u : 0u);
+    return m ? q * wtab[S] : 0u;
+  };
+  const uint32_t wI0 = weight(mI0, qI0, 0), wI1 = weight(mI1, qI1, 1);
+  const uint32_t wO0 = weight(mO0, qO0, 2), wO1 = weight(mO1, qO1, 3);
+  const uint32_t wO2 = weight(mO2, qO2, 4), wO3 = weight(mO3, qO3, 5);
+  // D7 moments in the lane frame, then rotated (cs*sn = 0)
+  const uint32_t wO = wO0 + wO1 + wO2 + wO3, wI = wI0 + wI1;
+  uint32_t Wsum = wI + wO;
+  const int32_t Ma = int32_t(wI + 2u * wO);
+  const int32_t Mb = int32_t(wI1 + wO2 + 2u * wO3) - int32_t(wO0);
+  const uint32_t Maa = wI + 4u * wO;
+  const uint32_t Mbb = wI1 + wO0 + wO2 + 4u * wO3;
+  int32_t Mp = cs * Ma - sn * Mb, Mt = sn * Ma + cs * Mb;
+  uint32_t Mpp = cs ? Maa : Mbb, Mtt = cs ? Mbb : Maa;
+#pragma unroll
+  for (int o = 1; o <= 2; o <<= 1) {
+    Wsum += __shfl_xor_sync(0xffffffffu, Wsum, o);
+    Mp += __shfl_xor_sync(0xffffffffu, Mp, o);
+    Mt += __shfl_xor_sync(0xffffffffu, Mt, o);
+    Mpp += __shfl_xor_sync(0xffffffffu, Mpp, o);
+    Mtt += __shfl_xor_sync(0xffffffffu, Mtt, o);
+    meta += __shfl_xor_sync(0xffffffffu, meta, o);
+  }
+  Wsum += qP * kShareL;                                                 // D6: w(P) = L Q(P)
+  uint32_t flags = 0;
+  if (pad < 2u || pad + 2u >= npads) flags |= 1u;                       // D8 EDGE_PAD
+  if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
+  if (qP == kQClamp || (meta & 0xFF00u)) flags |= 4u;                   // SATURATED
+  if (meta >> 16) flags |= 8u;                                          // SPLIT
+  lo = make_uint4(sector | (row << 8) | (pad << 16) | (flags << 24), uint32_t(tglob),
+                  qP | (((meta & 0xFFu) + 1u) << 16), Wsum);
+  hi = make_uint4(uint32_t(Mp), uint32_t(Mt), Mpp, Mtt);
+}
+
+// ----------------------------------------------------------------------------------------
+// S5 finish (D8): RawRec -> ClusterRec in place, one thread per record.  Evaluated in double
+// from the exact integers and rounded once to float32.
+// ----------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_finish(void* __restrict__ out, uint64_t out_capacity,
+                                                const DevStatus* __restrict__ status) {
+  const unsigned long long nc = status->n_clusters;
+  const uint64_t n = nc < out_capacity ? nc : out_capacity;
+  uint4* o = reinterpret_cast<uint4*>(out);
+  for (uint64_t i = uint64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += uint64_t(gridDim.x) * blockDim.x) {
+    uint4 lo = o[2 * i], hi = o[2 * i + 1];
+    const uint32_t W_ = lo.w;
+    const int32_t Mp = int32_t(hi.x), Mt = int32_t(hi.y);
+    const double Wd = double(W_);
+    const long long Np = (long long)hi.z * (long long)W_ - (long long)Mp * (long long)Mp;
+    const long long Nt = (long long)hi.w * (long long)W_ - (long long)Mt * (long long)Mt;
+    lo.w = __float_as_uint(float(Wd / 40320.0));
+    hi.x = __float_as_uint(float(double(Mp) / Wd));
+    hi.y = __float_as_uint(float(double(Mt) / Wd));
+    hi.z = __float_as_uint(float(sqrt(double(Np)) / Wd));
+    hi.w = __float_as_uint(float(sqrt(double(Nt)) / Wd));
+    o[2 * i] = lo;
+    o[2 * i + 1] = hi;
+  }
 }
 
 // D4 on the smem map for the digit (pad, tl, q): strictly greater than the 4 neighbours earlier
@@ -601,17 +654,35 @@ __device__ __forceinline__ bool is_peak(const uint32_t* __restrict__ map32, uint
   return q > early && q >= late;
 }
 
+// Worker / committer pipeline.  Warps 0..6 (the workers) take tiles by ticket and run S1..S5
+// on them; the RawRecs of a tile are written to one of two shared-memory staging buffers and
+// handed to warp 7 (the committer), which runs the decoupled look-back of the tile (S6) and
+// copies the records to their final position while the workers are already on the next tile.
+// Hand-over is by named barriers (bar.arrive / bar.sync, 256 participants each):
+//   kBarFull + b   workers arrive, committer syncs : staging[b] and meta[b] are written
+//   kBarEmpty + b  committer arrives, workers sync : staging[b] has been copied out
+// A tile with more peaks than the staging buffer holds is handed over in several items.
+constexpr int kBarWork = 1, kBarFull = 2, kBarEmpty = 4;
+constexpr uint32_t kStopTile = 0xFFFFFFFFu;
+__device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ TileParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
   uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   uint32_t* lbuf = reinterpret_cast<uint32_t*>(sp);         sp += kDigCap * 4;   // TMA bulk destination
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
+  uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
   uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += 16;
   uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // [0] tile, [1] digits (next tile)
-  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // [0] exclusive prefix, [1..8] warp totals
+  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // [1..7] warp totals, [12] next peak group
+  uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
   uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
   uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
+  uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;
+  uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 12 * 4;        // D6: L / S for S = 1..9
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t bmw = P.bm_words;
@@ -619,8 +690,36 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
     mbar_init(mbar, 1);
     fence_mbar_init();
   }
+  for (uint32_t i = tid; i < uint32_t(kNbrTabWords); i += kThreads) nbr_tab[i] = nbr_tab_entry(i);
+  if (tid < 9u) wtab[tid] = kShareL / (tid + 1u);
   __syncthreads();
 
+  if (warp == uint32_t(kWorkThreads / 32)) {
+    // ================= committer warp: S6 look-back + copy-out =================
+    uint32_t excl = 0;
+    for (uint32_t q = 0;; ++q) {
+      const uint32_t b = q & 1u;
+      bar_sync_named(kBarFull + int(b), kThreads);
+      const uint32_t t = s_meta[4 * b];
+      if (t == kStopTile) break;
+      const uint32_t total = s_meta[4 * b + 1], off = s_meta[4 * b + 2], cnt = s_meta[4 * b + 3];
+      if (off == 0u) {
+        excl = lookback_exclusive(P.tile_state, t, P.epoch, total);
+        if (lane == 0 && t == P.n_tiles - 1) P.status->n_clusters = (unsigned long long)excl + total;
+      }
+      const uint64_t g0 = uint64_t(excl) + off;                          // first record of this item
+      const uint4* src = stage + b * (2u * kListCap);
+      uint4* dst = reinterpret_cast<uint4*>(P.out) + 2 * g0;
+      for (uint32_t k = lane; k < 2u * cnt; k += 32u)
+        if (g0 + (k >> 1) < P.out_capacity) dst[k] = src[k];
+      bar_arrive_named(kBarEmpty + int(b), kThreads);
+    }
+    return;
+  }
+
+  // ================= worker warps =================
+  const uint32_t sub = lane & 3u;                                      // build phase: lane frame R_sub
+  const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
   // address and (clamped) length of a tile's digit list
   auto tile_list = [&](uint32_t t, const uint32_t*& src) -> uint32_t {
     const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
@@ -647,10 +746,10 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
     s_next[0] = t;
     s_next[1] = n;
   };
-  if (tid == kBuildThreads) fetch();
-  __syncthreads();
+  if (tid == 0) fetch();
+  bar_sync_named(kBarWork, kWorkThreads);
 
-  uint32_t parity = 0;
+  uint32_t parity = 0, q = 0;                                          // q: hand-over items issued so far
   for (;;) {
     const uint32_t t = s_next[0], n = s_next[1];
     if (t >= P.n_tiles) break;
@@ -669,25 +768,25 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
     {
       const uint32_t nz = (uint32_t(kBoxH) * W * 2u + uint32_t(kBoxH) * bmw * 4u + 15u) >> 4;
       uint4* z = reinterpret_cast<uint4*>(mapraw);
-      for (uint32_t i = tid; i < nz; i += kThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+      for (uint32_t i = tid; i < nz; i += kWorkThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
-    __syncthreads();
+    bar_sync_named(kBarWork, kWorkThreads);
 
     // ---- S1: scatter the staged digits into the map ----
     for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
       const uint32_t m = min(n - c0, uint32_t(kDigCap));
       if (c0) {
-        __syncthreads();
-        if (tid == kBuildThreads) issue(src, c0, m);
+        bar_sync_named(kBarWork, kWorkThreads);
+        if (tid == 0) issue(src, c0, m);
       }
       mbar_wait(mbar, parity);
       parity ^= 1u;
-      for (uint32_t i = tid; i < m; i += kThreads) {
+      for (uint32_t i = tid; i < m; i += kWorkThreads) {
         const uint32_t d = lbuf[i];
         map[dig_tl(d) * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));
       }
     }
-    __syncthreads();
+    bar_sync_named(kBarWork, kWorkThreads);
 
     // ---- S2: D4 peak flags for map rows 1..136, digit-driven ----
     {
@@ -695,22 +794,23 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
         const uint32_t m = min(n - c0, uint32_t(kDigCap));
         if (n > uint32_t(kDigCap)) {                                     // re-stage (the first pass overwrote lbuf)
-          __syncthreads();
-          if (tid == kBuildThreads) issue(src, c0, m);
+          bar_sync_named(kBarWork, kWorkThreads);
+          if (tid == 0) issue(src, c0, m);
           mbar_wait(mbar, parity);
           parity ^= 1u;
         }
-        for (uint32_t i = tid; i < m; i += kThreads) {
+        for (uint32_t i = tid; i < m; i += kWorkThreads) {
           const uint32_t d = lbuf[i];
-          const uint32_t q = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
-          if (q >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q))
+          const uint32_t q16 = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
+          if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
             atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
         }
       }
     }
-    __syncthreads();   // flags complete; lbuf is free
+    bar_sync_named(kBarWork, kWorkThreads);   // flags complete; lbuf is free
+    if (tid == 0) fetch();                    // next tile's ticket; its list lands during count + build
 
-    // ---- S6: ordered count of the core rows, block scan ----
+    // ---- S6 (in-tile part): ordered count of the core rows, block scan ----
     uint32_t cnt = 0;
     if (tid < ncore) {
       const uint32_t* r = bm + (kReach + tid) * bmw;
@@ -723,80 +823,85 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       if (lane >= uint32_t(o)) incl += v;
     }
     if (lane == 31) s_misc[1 + warp] = incl;
-    __syncthreads();
+    bar_sync_named(kBarWork, kWorkThreads);
     uint32_t wbase = 0, total = 0;
 #pragma unroll
-    for (int w = 0; w < kThreads / 32; ++w) {
+    for (int w = 0; w < kWorkThreads / 32; ++w) {
       const uint32_t v = s_misc[1 + w];
       if (uint32_t(w) < warp) wbase += v;
       total += v;
     }
     if (tid <= kTileT) rowoff[tid] = (tid < kTileT) ? (wbase + incl - cnt) : total;
+    // publish the tile's count early so that later tiles' look-backs never wait for this tile's build
+    if (tid == 0 && t != 0u) st_release_u64(P.tile_state + t, pack_state(P.epoch, kStAgg, total));
 
-    if (warp == kBuildThreads / 32) {
-      // ---- dedicated warp: next tile's ticket + list staging, then the look-back of this tile ----
-      if (lane == 0) fetch();
-      const uint32_t excl = lookback_exclusive(P.tile_state, t, P.epoch, total);
-      if (lane == 0) {
-        s_misc[0] = excl;
-        if (t == P.n_tiles - 1) P.status->n_clusters = (unsigned long long)excl + total;
-      }
-    } else {
-      // ---- S3..S5: clusters, kListCap peaks per pass, by warps 0..6 ----
-      for (uint32_t done = 0; done < total;) {
-        // rows whose peaks fit in the list: rowoff[r] + cnt - done <= kListCap
-        // (a row holds at most 124 peaks, so every pass makes progress)
-        if (tid < ncore) {
-          const uint32_t ro = rowoff[tid], rn = ro + cnt;
-          if (ro >= done && rn - done <= kListCap && cnt) {
-            uint32_t k = ro - done;
-            const uint32_t* r = bm + (kReach + tid) * bmw;
-            for (uint32_t w = 0; w < bmw; ++w) {
-              uint32_t bits = r[w];
-              while (bits) {
-                const uint32_t b = __ffs(bits) - 1;
-                bits &= bits - 1;
-                plist[k++] = ((kReach + tid) << 16) | (w * 32 + b - 4);    // (map row, pad)
-              }
+    // ---- S3..S5: clusters, at most kListCap peaks per hand-over item ----
+    uint32_t done = 0;
+    do {
+      const uint32_t b = q & 1u;
+      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
+      // rows whose peaks fit in this item: rowoff[r] + cnt - done <= kListCap (a row holds < kListCap peaks)
+      if (tid < ncore) {
+        const uint32_t ro = rowoff[tid], rn = ro + cnt;
+        if (ro >= done && rn - done <= kListCap && cnt) {
+          uint32_t k = ro - done;
+          const uint32_t* r = bm + (kReach + tid) * bmw;
+          for (uint32_t w = 0; w < bmw; ++w) {
+            uint32_t bits = r[w];
+            while (bits) {
+              const uint32_t bb = __ffs(bits) - 1;
+              bits &= bits - 1;
+              plist[k++] = ((kReach + tid) << 16) | (w * 32 + bb - 4);   // (map row, pad)
             }
           }
         }
-        bar_sync_named(1, kBuildThreads);
-        // number of peaks in this pass = largest rowoff[r] - done that is <= kListCap
-        uint32_t npass = min(total - done, uint32_t(kListCap));
-        if (total - done > kListCap) {
-          uint32_t lo = 0, hi = ncore;               // rowoff is non-decreasing
-          while (hi - lo > 1) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (rowoff[mid] - done <= kListCap && rowoff[mid] >= done) lo = mid; else hi = mid;
-          }
-          npass = (rowoff[hi] >= done && rowoff[hi] - done <= kListCap) ? rowoff[hi] - done : rowoff[lo] - done;
-        }
-        // first wave: one record per thread, built while the look-back is still running
-        ClusterRec rec;
-        const bool have = tid < npass;
-        if (have) {
-          const uint32_t e = plist[tid];
-          build_cluster(map, bm, W, bmw, e >> 16, e & 0xFFFFu, sector, row, ri.npads,
-                        t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, rec);
-        }
-        if (done == 0) bar_sync_named(2, kThreads);  // look-back result (the dedicated warp arrives below)
-        const uint64_t gbase = uint64_t(s_misc[0]) + done;
-        if (have && gbase + tid < P.out_capacity) store_rec(P.out, gbase + tid, rec);
-        for (uint32_t i = tid + kBuildThreads; i < npass; i += kBuildThreads) {
-          if (gbase + i < P.out_capacity) {
-            const uint32_t e = plist[i];
-            build_cluster(map, bm, W, bmw, e >> 16, e & 0xFFFFu, sector, row, ri.npads,
-                          t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, rec);
-            store_rec(P.out, gbase + i, rec);
-          }
-        }
-        done += npass;
-        bar_sync_named(1, kBuildThreads);            // plist is rewritten by the next pass
       }
-    }
-    if (warp == kBuildThreads / 32 && total) bar_sync_named(2, kThreads);   // pairs with the "done == 0" barrier above
-    __syncthreads();   // map, bitmap and s_next are stable until here
+      if (tid == 0) s_misc[12] = 0u;
+      bar_sync_named(kBarWork, kWorkThreads);
+      // peaks of this item: all that are left, or the longest prefix of whole rows that fits
+      uint32_t npass = total - done;
+      if (npass > uint32_t(kListCap)) {
+        uint32_t lo = 0, hi = ncore + 1u;            // rowoff[0..ncore] is non-decreasing, rowoff[ncore] = total
+        while (hi - lo > 1) {                        // largest row boundary <= done + kListCap
+          const uint32_t mid = (lo + hi) >> 1;
+          if (rowoff[mid] <= done + uint32_t(kListCap)) lo = mid; else hi = mid;
+        }
+        npass = rowoff[lo] - done;
+      }
+      if (tid == 0) {
+        s_meta[4 * b] = t;
+        s_meta[4 * b + 1] = total;
+        s_meta[4 * b + 2] = done;
+        s_meta[4 * b + 3] = npass;
+      }
+      // groups of 8 peaks, four lanes per peak, taken dynamically by the worker warps
+      uint4* stg = stage + b * (2u * kListCap);
+      for (;;) {
+        uint32_t g = 0;
+        if (lane == 0) g = atomicAdd(&s_misc[12], 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g * 8u >= npass) break;
+        const uint32_t i = g * 8u + (lane >> 2);
+        const uint32_t e = plist[min(i, npass - 1u)];
+        uint4 lo4, hi4;
+        build_cluster4(map, bm, nbr_tab, wtab, W, bmw, e >> 16, e & 0xFFFFu, sub, rot_cs, rot_sn, sector, row,
+                       ri.npads, t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, lo4, hi4);
+        if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
+      }
+      bar_arrive_named(kBarFull + int(b), kThreads);
+      ++q;
+      done += npass;
+      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // plist and s_misc[12] are reused
+    } while (done < total);
+    bar_sync_named(kBarWork, kWorkThreads);   // map, bitmap and s_next are stable until here
+  }
+  // stop item, then wait until the committer has drained the last real item
+  {
+    const uint32_t b = q & 1u;
+    if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);
+    if (tid == 0) s_meta[4 * b] = kStopTile;
+    bar_arrive_named(kBarFull + int(b), kThreads);
+    if (q >= 1u) bar_sync_named(kBarEmpty + int((q - 1u) & 1u), kThreads);
   }
 }
 
