@@ -31,6 +31,7 @@ struct tpcclus_ctx {
   uint32_t max_tiles = 0;
   uint32_t map_bytes_max = 0, bm_words = 0, smem_bytes = 0;
   int tile_grid = 0;              // persistent grid of k_tile
+  int bin_ctas_per_sm = 1;        // resident k_bin CTAs per SM (occupancy query)
   bool bin_aggregated = false;    // k_bin (CTA-aggregated) usable for this geometry, else k_bin_direct
   int n_sm = 0;
   uint32_t epoch = 0;
@@ -224,6 +225,12 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     if (c->bin_aggregated &&
         cudaFuncSetAttribute(k_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bin_smem_bytes(nb_max))) != cudaSuccess)
       return fail(TPCCLUS_ERR_CUDA);
+    if (c->bin_aggregated) {
+      int bocc = 0;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bocc, k_bin, kBinThreads, bin_smem_bytes(nb_max)) != cudaSuccess || bocc < 1)
+        return fail(TPCCLUS_ERR_CUDA);
+      c->bin_ctas_per_sm = bocc;
+    }
   }
 
   if (g->options & TPCCLUS_OPT_HOST_STAGING) {
@@ -309,7 +316,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
       bp.chunks_per_sector = uint32_t(cps);
       bp.pad_ = 0;
       const uint64_t total = uint64_t(g.n_sectors) * cps;
-      const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(total, 1), uint64_t(c->n_sm)));
+      const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(total, 1), uint64_t(c->n_sm) * c->bin_ctas_per_sm));
       k_bin<<<blocks, kBinThreads, bin_smem_bytes(bp.nb), st>>>(bp, c->d_rows, c->d_lists, c->d_counts, c->d_status);
     } else {
       const uint64_t pairs = (n + 1) / 2;

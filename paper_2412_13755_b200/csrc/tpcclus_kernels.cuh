@@ -258,36 +258,47 @@ __global__ void __launch_bounds__(256) k_bin_direct(const uint2* __restrict__ di
 // Why: with one global atomic per list entry (k_bin_direct) the kernel is bound by the L2
 // atomic units — all CTAs hammer the ~5000 contiguous counters of the sector being read
 // (profiles/r1b_bin_tile_ncu.md, 5.7 ms for 3.4e8 atomics).  Here a CTA takes a CHUNK of
-// 16384 digits of ONE sector, staged in shared memory by TMA bulk copies that land while the
-// previous chunk is still being written out, ranks every digit inside its bin with a
-// shared-memory atomic, reserves the chunk's slots with ONE global atomic per non-empty bin,
-// and then stores the packed digits.  Chunks are dealt round-robin over the sectors so that
-// concurrently running CTAs reserve in different sectors' counters.
+// kBinChunk digits of ONE sector, staged in shared memory by TMA bulk copies, and works on it
+// IN PLACE in three barrier-separated phases:
+//   1  quantise (D1), validate, rank every digit inside its bin with a shared-memory atomic;
+//      the 8-byte digit is overwritten by (packed list entry, bin | rank << 14).  A digit within
+//      5 bins of a tile seam also belongs to the next tile: that second entry goes to a small
+//      overflow list (direct global path when the list is full).
+//   2  one global reservation per non-empty bin (batched, so the atomics' latencies overlap)
+//   3  store the packed digits at reservation + rank
+// No per-thread state survives a barrier, so the kernel needs few registers and two CTAs share
+// an SM: one CTA's TMA wait and reservation latency hide behind the other's ranking and stores.
+// Chunks are dealt round-robin over the sectors so that concurrently running CTAs reserve in
+// different sectors' counters.
 // ----------------------------------------------------------------------------------------
 constexpr int      kBinThreads  = 1024;
-constexpr int      kBinPer      = 16;                       // digits per thread per chunk
-constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 16384 digits = 128 KB of input
-constexpr uint32_t kBinMaxNb    = 16384;                    // bins per sector the histogram can hold
+constexpr int      kBinPer      = 8;                        // digits per thread per chunk
+constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 8192 digits = 64 KB of input
+constexpr int      kBinOvfCap   = 1536;                     // second-tile entries kept in shared memory per chunk
+constexpr uint32_t kBinMaxNb    = 16384;                    // bins per sector the histogram can hold (14-bit bin id)
 constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room for this chunk (duplicates only)
+constexpr uint32_t kBinNone     = 0xFFFFFFFFu;              // stage entry without a list entry
 constexpr int      kTileShift   = 7;
 static_assert((1 << kTileShift) == kTileT, "tile size is a power of two");
+static_assert(2 * kBinChunk <= (1 << 15), "rank fits 15 bits");
 
 __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
-  return uint32_t(kBinChunk) * 8u + ((nb + 3u) & ~3u) * 4u + 3u * 256u * 4u + 64u;
+  return uint32_t(kBinChunk) * 8u + ((nb + 3u) & ~3u) * 4u + uint32_t(kBinOvfCap) * 8u + 3u * 256u * 4u + 64u + 128u;
 }
 
-__global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ BinParams P,
+__global__ void __launch_bounds__(kBinThreads, 2) k_bin(const __grid_constant__ BinParams P,
                                                         const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
                                                         uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-  const uint4* stage = reinterpret_cast<const uint4*>(sp);   sp += uint32_t(kBinChunk) * 8u;   // TMA destination
+  uint2* stage = reinterpret_cast<uint2*>(sp);                sp += uint32_t(kBinChunk) * 8u;   // TMA destination, then work area
   uint32_t* hist = reinterpret_cast<uint32_t*>(sp);           sp += ((P.nb + 3u) & ~3u) * 4u;
+  uint2* ovf = reinterpret_cast<uint2*>(sp);                  sp += uint32_t(kBinOvfCap) * 8u;
   uint32_t* r_npads = reinterpret_cast<uint32_t*>(sp);        sp += 256 * 4;
   uint32_t* r_off = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint32_t* r_cap = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);           sp += 16;
-  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);         sp += 16;
+  uint32_t* s_ovf = reinterpret_cast<uint32_t*>(sp);          sp += 16;
 
   const uint32_t tid = threadIdx.x;
   for (uint32_t i = tid; i < 256u; i += kBinThreads) {
@@ -328,107 +339,115 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     np = uint32_t(min(uint64_t(kPairs), p1 - pa));
     return true;
   };
-  // one thread: find the next non-empty chunk at or after k (stride gridDim.x), start its TMA
-  auto fetch = [&](uint32_t k) {
-    uint32_t s = 0, np = 0;
-    uint64_t pa = 0;
-    while (k < total && !chunk(k, s, pa, np)) k += gridDim.x;
-    if (k < total) {
-      mbar_arrive_expect_tx(mbar, np * 16u);
-      for (uint32_t o = 0; o < np; o += 2048u)            // <= 32 KB per bulk copy
-        tma_bulk_load(const_cast<uint4*>(stage) + o, P.base16 + pa + o, min(2048u, np - o) * 16u, mbar);
-    }
-    s_next[0] = k;
-  };
-  __syncthreads();
-  if (tid == 0) fetch(blockIdx.x);
+  const int32_t tpr = int32_t(P.tiles_per_row);
   __syncthreads();
 
   uint32_t parity = 0;
-  for (;;) {
-    const uint32_t k = s_next[0];
-    if (k >= total) break;
+  for (uint32_t k = blockIdx.x; k < total; k += gridDim.x) {
     uint32_t s, np;
     uint64_t pa;
-    chunk(k, s, pa, np);
-    const uint64_t d_lo = P.off[s], d_hi = P.off[s + 1];     // digits of this sector
+    if (!chunk(k, s, pa, np)) continue;                      // uniform over the CTA
+    if (tid == 0) {
+      // the staging area was last written through the generic proxy (phase 1 of the previous chunk)
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_arrive_expect_tx(mbar, np * 16u);
+      for (uint32_t o = 0; o < np; o += 2048u)               // <= 32 KB per bulk copy
+        tma_bulk_load(reinterpret_cast<uint4*>(stage) + o, P.base16 + pa + o, min(2048u, np - o) * 16u, mbar);
+      s_ovf[0] = 0u;
+    }
     for (uint32_t i = tid; i < P.nb; i += kBinThreads) hist[i] = 0u;
+    // slots [slot_lo, slot_hi) of the chunk hold digits of sector s (slot j = digit first + j)
+    uint32_t slot_lo, slot_hi;
+    {
+      const int64_t first = int64_t(2ull * pa) - int64_t(P.head);
+      slot_lo = uint32_t(max(int64_t(P.off[s]) - first, int64_t(0)));
+      slot_hi = uint32_t(min(int64_t(P.off[s + 1]) - first, int64_t(2u * np)));
+    }
+    const uint32_t cbase = s * P.nb;
+    uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
     __syncthreads();
     mbar_wait(mbar, parity);
     parity ^= 1u;
 
-    // ---- phase 1: quantise (D1), validate, rank inside the bin (shared-memory atomics) ----
-    uint32_t pk[kBinPer];            // packed digit for its first tile
-    uint32_t br[kBinPer];            // bin | rank << 14 | second-tile << 29 | valid << 30
-    uint32_t r2[kBinPer / 2];        // ranks in the second tile, two per word
-#pragma unroll
-    for (int j = 0; j < kBinPer / 2; ++j) {
-      const uint32_t pi = uint32_t(j) * kBinThreads + tid;
-      uint4 v = make_uint4(0u, 0u, 0u, 0u);
-      if (pi < np) v = stage[pi];
-      const uint64_t i0 = 2ull * (pa + pi) - P.head;         // digit index of the low slot
-      r2[j] = 0u;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const uint32_t w0 = h ? v.z : v.x, w1 = h ? v.w : v.y;
-        const uint64_t idx = i0 + uint64_t(h);
-        uint32_t pkv = 0u, brv = 0u;
-        if (pi < np && idx >= d_lo && idx < d_hi) {
-          const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
-          const int32_t time = int32_t(w0 >> 16);
-          const uint32_t q = quantise_q16(__uint_as_float(w1));
-          if (q == 0u || time < P.t_lo || time >= P.t_hi || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
-            ++dropped;
-          } else {
-            const int32_t u = time - P.t_core_begin;
-            const int32_t tlo = max((u - kReach) >> kTileShift, 0);
-            const int32_t thi = min((u + kReach) >> kTileShift, int32_t(P.tiles_per_row) - 1);
-            if (tlo <= thi) {
-              const uint32_t bin = row * P.tiles_per_row + uint32_t(tlo);
-              pkv = pack_digit(pad, uint32_t(u - (tlo << kTileShift) + kReach), q);
-              brv = bin | (atomicAdd(&hist[bin], 1u) << 14) | (1u << 30);
-              if (thi != tlo) {
-                brv |= 1u << 29;
-                r2[j] |= atomicAdd(&hist[bin + 1u], 1u) << (16 * h);
+    // ---- phase 1: quantise (D1), validate, rank inside the bin; overwrite the digit in place ----
+#pragma unroll 4
+    for (int i = 0; i < kBinPer; ++i) {
+      const uint32_t j = uint32_t(i) * kBinThreads + tid;
+      uint2 e = make_uint2(0u, kBinNone);
+      if (j >= slot_lo && j < slot_hi) {
+        const uint2 v = stage[j];
+        const uint32_t row = v.x & 0xFFu, pad = (v.x >> 8) & 0xFFu;
+        const int32_t time = int32_t(v.x >> 16);
+        const uint32_t q = quantise_q16(__uint_as_float(v.y));
+        if (q == 0u || time < P.t_lo || time >= P.t_hi || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
+          ++dropped;
+        } else {
+          const int32_t u = time - P.t_core_begin;
+          const int32_t tlo = max((u - kReach) >> kTileShift, 0);
+          const int32_t thi = min((u + kReach) >> kTileShift, tpr - 1);
+          if (tlo <= thi) {
+            const uint32_t bin = row * uint32_t(tpr) + uint32_t(tlo);
+            e.x = pack_digit(pad, uint32_t(u - (tlo << kTileShift) + kReach), q);
+            e.y = bin | (atomicAdd(&hist[bin], 1u) << 14);
+            if (thi != tlo) {                                 // also in the next tile's window
+              const uint32_t pk2 = e.x - (uint32_t(kTileT) << 8);
+              const uint32_t k2 = atomicAdd(&s_ovf[0], 1u);
+              if (k2 < uint32_t(kBinOvfCap)) {
+                ovf[k2] = make_uint2(pk2, (bin + 1u) | (atomicAdd(&hist[bin + 1u], 1u) << 14));
+              } else {                                        // overflow list full: direct global path
+                const uint32_t cap = r_cap[row];
+                const uint32_t slot = atomicAdd(&counts[cbase + bin + 1u], 1u);
+                if (slot < cap) seclist[r_off[row] + uint32_t(tlo + 1) * cap + slot] = pk2;
               }
             }
           }
         }
-        pk[2 * j + h] = pkv;
-        br[2 * j + h] = brv;
       }
+      stage[j] = e;
     }
-    __syncthreads();                  // stage is consumed, hist is complete
+    __syncthreads();                  // every entry is ranked, hist is complete
 
-    // ---- phase 2: next chunk's TMA; one global reservation per non-empty bin ----
-    if (tid == 0) fetch(k + gridDim.x);
-    for (uint32_t b = tid; b < P.nb; b += kBinThreads) {
-      const uint32_t c = hist[b];
-      if (c) {
-        const uint32_t row = b / P.tiles_per_row, tt = b - row * P.tiles_per_row;
-        const uint32_t cap = r_cap[row];
-        const uint32_t base = atomicAdd(&counts[s * P.nb + b], c);
-        hist[b] = (base + c <= cap) ? r_off[row] + tt * cap + base : kBinFull;
+    // ---- phase 2: one global reservation per non-empty bin, four in flight per thread ----
+    for (uint32_t b0 = tid; b0 < P.nb; b0 += 4u * kBinThreads) {
+      uint32_t c[4], g[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const uint32_t b = b0 + uint32_t(u) * kBinThreads;
+        c[u] = b < P.nb ? hist[b] : 0u;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        g[u] = c[u] ? atomicAdd(&counts[cbase + b0 + uint32_t(u) * kBinThreads], c[u]) : 0u;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (c[u]) {
+          const uint32_t b = b0 + uint32_t(u) * kBinThreads;
+          const uint32_t row = b / uint32_t(tpr), tt = b - row * uint32_t(tpr);
+          const uint32_t cap = r_cap[row];
+          hist[b] = (g[u] + c[u] <= cap) ? r_off[row] + tt * cap + g[u] : kBinFull;
+        }
       }
     }
     __syncthreads();
 
-    // ---- phase 3: store the packed digits at base + rank ----
-    uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
-#pragma unroll
+    // ---- phase 3: store the packed digits at reservation + rank ----
+#pragma unroll 4
     for (int i = 0; i < kBinPer; ++i) {
-      const uint32_t b = br[i];
-      if (b & (1u << 30)) {
-        const uint32_t bin = b & 0x3FFFu;
-        const uint32_t e = hist[bin];
-        if (e != kBinFull) seclist[e + ((b >> 14) & 0x7FFFu)] = pk[i];
-        if (b & (1u << 29)) {
-          const uint32_t e2 = hist[bin + 1u];
-          if (e2 != kBinFull) seclist[e2 + ((r2[i >> 1] >> (16 * (i & 1))) & 0xFFFFu)] = pk[i] - (uint32_t(kTileT) << 8);
-        }
+      const uint2 e = stage[uint32_t(i) * kBinThreads + tid];
+      if (e.y != kBinNone) {
+        const uint32_t d = hist[e.y & 0x3FFFu];
+        if (d != kBinFull) seclist[d + (e.y >> 14)] = e.x;
       }
     }
-    __syncthreads();                  // hist and s_next are stable until here
+    {
+      const uint32_t novf = min(s_ovf[0], uint32_t(kBinOvfCap));
+      for (uint32_t i = tid; i < novf; i += kBinThreads) {
+        const uint2 e = ovf[i];
+        const uint32_t d = hist[e.y & 0x3FFFu];
+        if (d != kBinFull) seclist[d + (e.y >> 14)] = e.x;
+      }
+    }
+    __syncthreads();                  // stage, hist and the overflow list are reused by the next chunk
   }
   dropped = __reduce_add_sync(0xffffffffu, dropped);
   if ((tid & 31u) == 0u && dropped) atomicAdd(&status->n_dropped, (unsigned long long)dropped);
