@@ -26,7 +26,9 @@ struct tpcclus_ctx {
   std::vector<uint16_t> npads;
   std::vector<RowInfo> rows;
   int device = 0;
-  uint32_t tiles_per_row_max = 0; // bins laid out per (sector,row): ceil(max_core_bins / kTileT)
+  uint32_t tiles_per_row_max = 0; // ceil(max_core_bins / kTileT)
+  uint32_t bins_per_row_max = 0;  // digit bins laid out per (sector,row): ceil(max_core_bins / kBinT)
+  uint32_t max_bins = 0;
   uint64_t sec_list_elems = 0;    // digit-list elements per sector
   uint32_t max_tiles = 0;
   uint32_t map_bytes_max = 0, bm_words = 0, smem_bytes = 0;
@@ -167,9 +169,13 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (prop.major < 10) return fail(TPCCLUS_ERR_CUDA);       // TMA + sm_100a code only; no fallback
   c->n_sm = prop.multiProcessorCount;
 
-  // geometry tables: one digit bin per (sector, row, 128-bin time tile), one slot per map cell
+  // geometry tables: one digit bin per (sector, row, kBinT time bins).  Capacity: 5/4 slots per
+  // cell of the bin's window (D2: at most one digit per cell; the rest absorbs the zero padding of
+  // k_bin's whole-sector flushes: < 16 entries per CTA and bin, and 7 per reserve-8 append)
   c->tiles_per_row_max = (g->max_core_bins + kTileT - 1) / kTileT;
-  const uint32_t bin_rows = std::min<uint32_t>(uint32_t(kBoxH), g->max_core_bins + 2 * g->halo_bins);
+  c->bins_per_row_max = (g->max_core_bins + kBinT - 1) / kBinT;
+  const uint32_t bin_rows = std::min<uint32_t>(uint32_t(kBinBoxH), g->max_core_bins + 2 * g->halo_bins);
+  const uint32_t cap_margin = 16u * uint32_t(c->n_sm) + 64u;
   c->rows.resize(g->n_rows);
   uint64_t off = 0;
   uint32_t max_W = 0, max_npads = 0;
@@ -177,11 +183,11 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     RowInfo& ri = c->rows[r];
     ri.npads = c->npads[r];
     ri.W = uint16_t(roundup(ri.npads + 2 * kColOff, 8));
-    ri.cap = roundup(bin_rows * ri.npads, 4);
+    ri.cap = roundup(bin_rows * ri.npads + bin_rows * ri.npads / 4 + cap_margin, 8);
     ri.pad_ = 0;
     if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
     ri.list_off = uint32_t(off);
-    off += uint64_t(c->tiles_per_row_max) * ri.cap;
+    off += uint64_t(c->bins_per_row_max) * ri.cap;
     max_W = std::max<uint32_t>(max_W, ri.W);
     max_npads = std::max<uint32_t>(max_npads, ri.npads);
   }
@@ -191,13 +197,14 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * c->tiles_per_row_max;
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
+  c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
   c->smem_bytes = kDigCap * 4 + c->map_bytes_max + 2 * kListCap * 32 + 16 + 16 + 16 * 4 + 2 * 4 * 4 + kListCap * 4 +
                   (kTileT + 4) * 4 + kNbrTabWords * 4 + 12 * 4 + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;
   if ((rc = dev_alloc(c, &c->d_lists, list_bytes)) != TPCCLUS_OK) return fail(rc);
-  if ((rc = dev_alloc(c, &c->d_counts, (uint64_t(c->max_tiles) + 4) * 4)) != TPCCLUS_OK) return fail(rc);
+  if ((rc = dev_alloc(c, &c->d_counts, (uint64_t(c->max_bins) + 4) * 4)) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_rows, g->n_rows * sizeof(RowInfo))) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_tile_state, uint64_t(c->max_tiles) * 8)) != TPCCLUS_OK) return fail(rc);
   if ((rc = dev_alloc(c, &c->d_status, sizeof(DevStatus))) != TPCCLUS_OK) return fail(rc);
@@ -219,7 +226,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     return fail(TPCCLUS_ERR_CUDA);
   c->tile_grid = occ * c->n_sm;
   {
-    const uint32_t nb_max = g->n_rows * c->tiles_per_row_max;
+    const uint32_t nb_max = g->n_rows * c->bins_per_row_max;
     c->bin_aggregated = nb_max <= kBinMaxNb && bin_smem_bytes(nb_max) <= uint32_t(prop.sharedMemPerBlockOptin) &&
                         !std::getenv("TPCCLUS_BIN_DIRECT");
     if (c->bin_aggregated &&
@@ -272,6 +279,8 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
 
   const uint32_t tiles_per_row = (e - b + kTileT - 1) / kTileT;
   const uint32_t n_tiles = g.n_sectors * g.n_rows * tiles_per_row;
+  const uint32_t bins_per_row = (e - b + kBinT - 1) / kBinT;
+  const uint32_t n_bins = g.n_sectors * g.n_rows * bins_per_row;
   c->epoch = (c->epoch + 1) & 0x3FFFFFFFu;
   if (c->epoch == 0) {   // wrapped: stale words could alias, so wipe them once
     CK(c, cudaMemsetAsync(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8, st));
@@ -280,8 +289,8 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
 
   // S0: counters + status
   {
-    const uint32_t blocks = std::min<uint32_t>((n_tiles / 4 + 256) / 256, uint32_t(c->n_sm) * 8);
-    k_init<<<std::max(blocks, 1u), 256, 0, st>>>(c->d_counts, n_tiles, c->d_status);
+    const uint32_t blocks = std::min<uint32_t>((n_bins / 4 + 256) / 256, uint32_t(c->n_sm) * 8);
+    k_init<<<std::max(blocks, 1u), 256, 0, st>>>(c->d_counts, n_bins, c->d_status);
     c->launches++;
     debug_check(st, "k_init");
     if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][1], st));
@@ -296,26 +305,27 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     bp.t_hi = int32_t(std::min<uint64_t>(g.tf_time_bins, uint64_t(e) + g.halo_bins));
     bp.n_sectors = g.n_sectors;
     bp.n_rows = g.n_rows;
-    bp.tiles_per_row = tiles_per_row;
-    bp.tiles_per_row_max = c->tiles_per_row_max;
+    bp.bins_per_row = bins_per_row;
+    bp.bins_per_row_max = c->bins_per_row_max;
     std::memcpy(bp.off, h_off, (g.n_sectors + 1) * sizeof(uint64_t));
-    bp.nb = g.n_rows * tiles_per_row;
+    bp.nb = g.n_rows * bins_per_row;
     if (c->bin_aggregated && bp.nb <= kBinMaxNb) {
       // CTA-aggregated binning: chunks of kBinChunk digits, one sector per chunk
       bp.head = (reinterpret_cast<uintptr_t>(d_digits) & 8u) ? 1u : 0u;
       bp.base16 = reinterpret_cast<const uint4*>(reinterpret_cast<uintptr_t>(d_digits) - 8u * bp.head);
       bp.pair_lo = bp.head;
       bp.pair_hi = (n + bp.head) >> 1;
-      uint64_t cps = 0;
+      uint32_t total = 0;
       for (uint32_t s = 0; s < g.n_sectors; ++s) {
+        bp.cpref[s] = total;
         if (h_off[s + 1] <= h_off[s]) continue;
         const uint64_t p0 = std::max<uint64_t>((h_off[s] + bp.head) >> 1, bp.pair_lo);
         const uint64_t p1 = std::min<uint64_t>((h_off[s + 1] + bp.head + 1) >> 1, bp.pair_hi);
-        if (p1 > p0) cps = std::max<uint64_t>(cps, (p1 - p0 + kBinChunk / 2 - 1) / (kBinChunk / 2));
+        if (p1 > p0) total += uint32_t((p1 - p0 + kBinChunk / 2 - 1) / (kBinChunk / 2));
       }
-      bp.chunks_per_sector = uint32_t(cps);
+      bp.cpref[g.n_sectors] = total;
+      bp.total_chunks = total;
       bp.pad_ = 0;
-      const uint64_t total = uint64_t(g.n_sectors) * cps;
       const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(total, 1), uint64_t(c->n_sm) * c->bin_ctas_per_sm));
       k_bin<<<blocks, kBinThreads, bin_smem_bytes(bp.nb), st>>>(bp, c->d_rows, c->d_lists, c->d_counts, c->d_status);
     } else {
@@ -342,7 +352,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     tp.n_sectors = g.n_sectors;
     tp.n_rows = g.n_rows;
     tp.tiles_per_row = tiles_per_row;
-    tp.tiles_per_row_max = c->tiles_per_row_max;
+    tp.bins_per_row = bins_per_row;
     tp.n_tiles = n_tiles;
     tp.t_core_begin = int32_t(b);
     tp.t_core_end = int32_t(e);

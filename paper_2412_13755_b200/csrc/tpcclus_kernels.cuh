@@ -30,6 +30,11 @@ constexpr int      kWorkThreads  = 224;   // warps 0..6 run S1..S5 on the tiles;
 constexpr int      kTileT        = 128;   // core time bins per tile
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
+constexpr int      kBinT         = 256;   // core time bins per digit bin (= two tiles: k_tile filters by half)
+constexpr int      kBinShift     = 8;
+constexpr int      kBinBoxH      = kBinT + 2 * kReach;    // time rows a bin's window spans (266)
+static_assert((1 << kBinShift) == kBinT && kBinT % kTileT == 0, "bins are whole tiles");
+constexpr int      kTilesPerBin  = kBinT / kTileT;
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
 constexpr int      kListCap      = 160;   // peaks per hand-over item (capacity of one staging buffer)
 constexpr int      kDigCap       = 4096;  // digits staged per TMA bulk copy (16 KB)
@@ -38,7 +43,7 @@ constexpr int      kMaxSectors   = 256;
 
 struct RowInfo {              // one per pad row (device table)
   uint32_t list_off;          // element offset of this row's bins inside one sector's digit lists
-  uint32_t cap;               // list capacity of one bin = roundup4(map rows * npads): one slot per cell
+  uint32_t cap;               // list capacity of one bin (multiple of 8): window cells * 5/4 + padding margin
   uint16_t npads;
   uint16_t W;                 // smem map pitch in cells = roundup8(npads + 4)
   uint32_t pad_;
@@ -57,16 +62,17 @@ struct BinParams {
   int32_t  t_core_begin;               // b
   int32_t  t_lo, t_hi;                 // loaded range [lo,hi) in global time (D1)
   uint32_t n_sectors, n_rows;
-  uint32_t tiles_per_row;              // tiles of this run
-  uint32_t tiles_per_row_max;          // bins laid out per (sector,row)
+  uint32_t bins_per_row;               // bins per (sector,row) of this run = ceil((e-b)/kBinT)
+  uint32_t bins_per_row_max;           // bins laid out per (sector,row)
   // k_bin (CTA-aggregated binning) only:
   const uint4* base16;                 // digit buffer aligned down to 16 bytes; digit i is 8-byte slot i + head
   uint32_t head;                       // 1 if the buffer starts in the upper half of a 16-byte pair
-  uint32_t nb;                         // bins per sector of this run = n_rows * tiles_per_row
-  uint32_t chunks_per_sector;          // max over sectors of ceil(pairs / (kBinChunk/2))
+  uint32_t nb;                         // bins per sector of this run = n_rows * bins_per_row
+  uint32_t total_chunks;               // cpref[n_sectors]
   uint32_t pad_;
   uint64_t pair_lo, pair_hi;           // pairs with both slots inside the buffer: [pair_lo, pair_hi)
   uint64_t off[kMaxSectors + 1];       // sector offsets (copied from the host array)
+  uint32_t cpref[kMaxSectors + 1];     // k_bin: chunks of sectors < s (sector s has ceil(pairs / (kBinChunk/2)) chunks)
 };
 
 struct TileParams {
@@ -80,7 +86,7 @@ struct TileParams {
   uint64_t           sec_list_elems;
   uint32_t n_sectors, n_rows;
   uint32_t tiles_per_row;              // ceil((e-b)/kTileT)
-  uint32_t tiles_per_row_max;
+  uint32_t bins_per_row;               // ceil((e-b)/kBinT)
   uint32_t n_tiles;
   int32_t  t_core_begin, t_core_end;   // [b,e)
   uint32_t tf_time_bins;
@@ -184,6 +190,21 @@ __device__ __forceinline__ uint32_t quantise_q16(float charge) {
   return x >= float(kQClamp) ? kQClamp : uint32_t(x);
 }
 
+// append one packed digit to a bin, reserving R slots (R = 1: k_bin_direct; R = 8: the odd
+// entries of the write-combining kernel, whose reservations stay multiples of 8 — the other
+// R-1 slots are zero = "no digit")
+template <int R>
+__device__ __forceinline__ void bin_append(uint32_t* __restrict__ seclist, uint32_t* __restrict__ cnt, uint32_t dest0,
+                                           uint32_t cap, uint32_t pk) {
+  const uint32_t slot = atomicAdd(cnt, uint32_t(R));
+  if (slot + uint32_t(R) <= cap) {
+    seclist[dest0 + slot] = pk;
+#pragma unroll
+    for (int x = 1; x < R; ++x) seclist[dest0 + slot + x] = 0u;
+  }
+}
+
+template <int R>
 __device__ __forceinline__ bool bin_one(uint32_t w0, uint32_t w1, uint64_t idx, uint32_t& sector,
                                         const BinParams& P, const RowInfo* srow, uint32_t* __restrict__ lists,
                                         uint32_t* __restrict__ counts) {
@@ -195,16 +216,13 @@ __device__ __forceinline__ bool bin_one(uint32_t w0, uint32_t w1, uint64_t idx, 
   const RowInfo ri = srow[row];
   if (pad >= ri.npads) return false;
   const int32_t u = time - P.t_core_begin;                       // >= -halo
-  int32_t tt_hi = (u + kReach) >> 7;                             // largest tt with 128 tt - 5 <= u
-  int32_t tt_lo = ((u - (kTileT + kReach)) >> 7) + 1;            // smallest tt with u < 128 tt + 133
-  tt_lo = max(tt_lo, 0);
-  tt_hi = min(tt_hi, int32_t(P.tiles_per_row) - 1);
-  const uint32_t sr = sector * P.n_rows + row;
-  const uint64_t base = uint64_t(sector) * P.sec_list_elems + ri.list_off;
-  for (int32_t tt = tt_lo; tt <= tt_hi; ++tt) {
-    const uint32_t tl = uint32_t(u - tt * kTileT + kReach);      // 0..137
-    const uint32_t slot = atomicAdd(&counts[sr * P.tiles_per_row + uint32_t(tt)], 1u);
-    if (slot < ri.cap) lists[base + uint64_t(tt) * ri.cap + slot] = pack_digit(pad, tl, q);
+  const int32_t tb_lo = max((u - kReach) >> kBinShift, 0);       // bins whose window [256 tb - 5, 256 tb + 261) holds u
+  const int32_t tb_hi = min((u + kReach) >> kBinShift, int32_t(P.bins_per_row) - 1);
+  uint32_t* seclist = lists + uint64_t(sector) * P.sec_list_elems;
+  for (int32_t tb = tb_lo; tb <= tb_hi; ++tb) {
+    const uint32_t tl = uint32_t(u - tb * kBinT + kReach);       // 0..265
+    bin_append<R>(seclist, &counts[(sector * P.n_rows + row) * P.bins_per_row + uint32_t(tb)],
+                  ri.list_off + uint32_t(tb) * ri.cap, ri.cap, pack_digit(pad, tl, q));
   }
   return true;
 }
@@ -238,14 +256,14 @@ __global__ void __launch_bounds__(256) k_bin_direct(const uint2* __restrict__ di
   for (uint64_t i = tid; i < npairs; i += stride) {
     const uint4 v = ld_stream_u4(pairs + i);
     const uint64_t idx = head + 2 * i;
-    dropped += bin_one(v.x, v.y, idx, sector, P, srow, lists, counts) ? 0u : 1u;
-    dropped += bin_one(v.z, v.w, idx + 1, sector, P, srow, lists, counts) ? 0u : 1u;
+    dropped += bin_one<1>(v.x, v.y, idx, sector, P, srow, lists, counts) ? 0u : 1u;
+    dropped += bin_one<1>(v.z, v.w, idx + 1, sector, P, srow, lists, counts) ? 0u : 1u;
   }
   if (tid == 0) {                                 // leftovers: the peeled head and an odd tail
     uint32_t s0 = 0;
-    if (head && n > 0) dropped += bin_one(digits[0].x, digits[0].y, 0, s0, P, srow, lists, counts) ? 0u : 1u;
+    if (head && n > 0) dropped += bin_one<1>(digits[0].x, digits[0].y, 0, s0, P, srow, lists, counts) ? 0u : 1u;
     const uint64_t tail = head + 2 * npairs;
-    if (tail < n) dropped += bin_one(digits[tail].x, digits[tail].y, tail, s0, P, srow, lists, counts) ? 0u : 1u;
+    if (tail < n) dropped += bin_one<1>(digits[tail].x, digits[tail].y, tail, s0, P, srow, lists, counts) ? 0u : 1u;
   }
   // warp-aggregated count of dropped digits
   dropped = __reduce_add_sync(0xffffffffu, dropped);
@@ -253,52 +271,61 @@ __global__ void __launch_bounds__(256) k_bin_direct(const uint2* __restrict__ di
 }
 
 // ----------------------------------------------------------------------------------------
-// S1 (first half), CTA-aggregated: the production binning kernel.
+// S1 (first half), write-combining: the production binning kernel.
 //
-// Why: with one global atomic per list entry (k_bin_direct) the kernel is bound by the L2
-// atomic units — all CTAs hammer the ~5000 contiguous counters of the sector being read
-// (profiles/r1b_bin_tile_ncu.md, 5.7 ms for 3.4e8 atomics).  Here a CTA takes a CHUNK of
-// kBinChunk digits of ONE sector, staged in shared memory by TMA bulk copies, and works on it
-// IN PLACE in three barrier-separated phases:
-//   1  quantise (D1), validate, rank every digit inside its bin with a shared-memory atomic;
-//      the 8-byte digit is overwritten by (packed list entry, bin | rank << 14).  A digit within
-//      5 bins of a tile seam also belongs to the next tile: that second entry goes to a small
-//      overflow list (direct global path when the list is full).
-//   2  one global reservation per non-empty bin (batched, so the atomics' latencies overlap)
-//   3  store the packed digits at reservation + rank
-// No per-thread state survives a barrier, so the kernel needs few registers and two CTAs share
-// an SM: one CTA's TMA wait and reservation latency hide behind the other's ranking and stores.
-// Chunks are dealt round-robin over the sectors so that concurrently running CTAs reserve in
-// different sectors' counters.
+// Why: appending digits one by one costs one scattered 4-byte store per list entry and, even
+// when a CTA aggregates a chunk's reservations, about one global atomic per 2-4 entries; ncu
+// shows both k_bin_direct and the chunk-aggregated variant pinned at ~45 % L1/L2 transaction
+// throughput with every warp waiting (profiles/r1c_*).  Here each CTA (one per SM) keeps an
+// 8-entry (32-byte = one DRAM sector) buffer per bin of the sector it is reading in shared
+// memory, and a bin costs ONE global atomic and ONE aligned 32-byte store per 8 entries:
+//   A   every digit of the chunk (TMA-staged, double-buffered): quantise (D1), validate, rank
+//       with a shared-memory atomic on the bin's fill count; ranks 0..7 go into the buffer, the
+//       thread that takes rank 7 queues the bin for flushing; the digit's slot in the staging
+//       area is overwritten by (entry, bin | rank << 12).  A digit within 5 bins of a bin seam
+//       also enters the next bin (second-entry list; reserve-8 direct path when that is full).
+//   B1  one thread per queued bin: reserve roundup8(count) slots with one global atomic, store
+//       the 8 buffered entries as one sector, zero-fill the padding, reset the count
+//   B2  entries that ranked >= 8 (more than a buffer's worth arrived within one chunk — rare
+//       for shuffled input, the rule for sorted input) are stored at reservation + rank
+// A CTA works through a contiguous range of chunks; buffers persist across the chunks of a
+// sector and are flushed (padded to 8 with zero = "no digit" entries) when the sector changes.
+// All reservations are multiples of 8, so every buffer flush is a 32-byte aligned store.
 // ----------------------------------------------------------------------------------------
 constexpr int      kBinThreads  = 1024;
-constexpr int      kBinPer      = 8;                        // digits per thread per chunk
-constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 8192 digits = 64 KB of input
-constexpr int      kBinOvfCap   = 1536;                     // second-tile entries kept in shared memory per chunk
-constexpr uint32_t kBinMaxNb    = 16384;                    // bins per sector the histogram can hold (14-bit bin id)
-constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room for this chunk (duplicates only)
-constexpr uint32_t kBinNone     = 0xFFFFFFFFu;              // stage entry without a list entry
-constexpr int      kTileShift   = 7;
-static_assert((1 << kTileShift) == kTileT, "tile size is a power of two");
-static_assert(2 * kBinChunk <= (1 << 15), "rank fits 15 bits");
+constexpr int      kBinPer      = 6;                        // digits per thread per chunk
+constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 6144 digits = 48 KB of input
+constexpr int      kBinSecCap   = 1024;                     // second (seam) entries kept per chunk
+constexpr uint32_t kBinMaxNb    = 4096;                     // bins per sector (12-bit bin id)
+constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room (duplicates only)
+constexpr uint32_t kBinNone     = 0xFFFFFFFFu;              // staging slot without a list entry
 
 __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
-  return uint32_t(kBinChunk) * 8u + ((nb + 3u) & ~3u) * 4u + uint32_t(kBinOvfCap) * 8u + 3u * 256u * 4u + 64u + 128u;
+  const uint32_t nb4 = (nb + 3u) & ~3u;
+  return 2u * uint32_t(kBinChunk) * 8u + nb4 * 32u + nb4 * 4u + nb4 * 4u + nb4 * 2u + uint32_t(kBinSecCap) * 8u +
+         3u * 256u * 4u + 96u + 128u;
 }
 
-__global__ void __launch_bounds__(kBinThreads, 2) k_bin(const __grid_constant__ BinParams P,
+__device__ __forceinline__ void st_v4(uint32_t* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
+
+__global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ BinParams P,
                                                         const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
                                                         uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
+  const uint32_t nb4 = (P.nb + 3u) & ~3u;
   uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-  uint2* stage = reinterpret_cast<uint2*>(sp);                sp += uint32_t(kBinChunk) * 8u;   // TMA destination, then work area
-  uint32_t* hist = reinterpret_cast<uint32_t*>(sp);           sp += ((P.nb + 3u) & ~3u) * 4u;
-  uint2* ovf = reinterpret_cast<uint2*>(sp);                  sp += uint32_t(kBinOvfCap) * 8u;
+  uint2* stage0 = reinterpret_cast<uint2*>(sp);               sp += 2u * uint32_t(kBinChunk) * 8u;   // two TMA destinations
+  uint32_t* buf = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 32u;     // 8 entries per bin
+  uint32_t* cnt = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // fill count per bin
+  uint2* sec = reinterpret_cast<uint2*>(sp);                  sp += uint32_t(kBinSecCap) * 8u;
   uint32_t* r_npads = reinterpret_cast<uint32_t*>(sp);        sp += 256 * 4;
   uint32_t* r_off = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint32_t* r_cap = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);           sp += 16;
-  uint32_t* s_ovf = reinterpret_cast<uint32_t*>(sp);          sp += 16;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);           sp += 16;            // one per staging buffer
+  uint32_t* s_ctl = reinterpret_cast<uint32_t*>(sp);          sp += 16;            // second entries of the chunk in staging buffer 0 / 1
+  uint32_t* s_par = reinterpret_cast<uint32_t*>(sp);          sp += 32;            // per staging buffer: sector, slot_lo, slot_hi
+  uint32_t* dst = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // list offset of the bin's last reservation
+  uint16_t* nfull = reinterpret_cast<uint16_t*>(sp);          sp += nb4 * 2u;      // whole sectors of that reservation
 
   const uint32_t tid = threadIdx.x;
   for (uint32_t i = tid; i < 256u; i += kBinThreads) {
@@ -307,9 +334,13 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_bin(const __grid_constant__ 
     r_off[i] = in ? rows[i].list_off : 0u;
     r_cap[i] = in ? rows[i].cap : 0u;
   }
+  for (uint32_t i = tid; i < P.nb; i += kBinThreads) cnt[i] = 0u;
   if (tid == 0) {
     mbar_init(mbar, 1);
+    mbar_init(mbar + 1, 1);
     fence_mbar_init();
+    s_ctl[0] = 0u;
+    s_ctl[1] = 0u;
   }
   uint32_t dropped = 0;
   // the (at most two) digits that do not sit in a full 16-byte pair: direct path, one thread
@@ -322,133 +353,202 @@ __global__ void __launch_bounds__(kBinThreads, 2) k_bin(const __grid_constant__ 
     for (int k = 0; k < ne; ++k) {
       uint32_t s0 = 0;
       const uint2 v = dg[edge[k]];
-      dropped += bin_one(v.x, v.y, edge[k], s0, P, rows, lists, counts) ? 0u : 1u;
+      dropped += bin_one<8>(v.x, v.y, edge[k], s0, P, rows, lists, counts) ? 0u : 1u;
     }
   }
 
   constexpr uint32_t kPairs = kBinChunk / 2;
-  const uint32_t total = P.n_sectors * P.chunks_per_sector;
-  // pair range of chunk k (sector k % n_sectors, chunk k / n_sectors of it); false if empty
-  auto chunk = [&](uint32_t k, uint32_t& s, uint64_t& pa, uint32_t& np) -> bool {
-    s = k % P.n_sectors;
-    const uint32_t ci = k / P.n_sectors;
+  // this CTA's contiguous range of chunks [k0, k1) of the sector-major chunk sequence
+  const uint32_t k0 = uint32_t(uint64_t(blockIdx.x) * P.total_chunks / gridDim.x);
+  const uint32_t k1 = uint32_t(uint64_t(blockIdx.x + 1) * P.total_chunks / gridDim.x);
+  // pair range of chunk k of sector s (k is the global chunk index)
+  auto chunk = [&](uint32_t k, uint32_t s, uint64_t& pa, uint32_t& np) {
     const uint64_t p0 = max((P.off[s] + P.head) >> 1, P.pair_lo);
     const uint64_t p1 = min((P.off[s + 1] + P.head + 1) >> 1, P.pair_hi);
-    pa = p0 + uint64_t(ci) * kPairs;
-    if (P.off[s + 1] <= P.off[s] || pa >= p1) return false;
+    pa = p0 + uint64_t(k - P.cpref[s]) * kPairs;
     np = uint32_t(min(uint64_t(kPairs), p1 - pa));
-    return true;
   };
-  const int32_t tpr = int32_t(P.tiles_per_row);
-  __syncthreads();
-
-  uint32_t parity = 0;
-  for (uint32_t k = blockIdx.x; k < total; k += gridDim.x) {
-    uint32_t s, np;
+  auto sector_of = [&](uint32_t k, uint32_t s) -> uint32_t {
+    while (k >= P.cpref[s + 1]) ++s;
+    return s;
+  };
+  // one thread: start the TMA copies of chunk k (sector s) into staging buffer b and leave the
+  // chunk's parameters for the CTA: slots [slot_lo, slot_hi) hold digits of sector s
+  auto load = [&](uint32_t k, uint32_t s, uint32_t b) {
     uint64_t pa;
-    if (!chunk(k, s, pa, np)) continue;                      // uniform over the CTA
-    if (tid == 0) {
-      // the staging area was last written through the generic proxy (phase 1 of the previous chunk)
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_arrive_expect_tx(mbar, np * 16u);
-      for (uint32_t o = 0; o < np; o += 2048u)               // <= 32 KB per bulk copy
-        tma_bulk_load(reinterpret_cast<uint4*>(stage) + o, P.base16 + pa + o, min(2048u, np - o) * 16u, mbar);
-      s_ovf[0] = 0u;
+    uint32_t np;
+    chunk(k, s, pa, np);
+    // the buffer was last written through the generic proxy (phase A two chunks ago)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    mbar_arrive_expect_tx(mbar + b, np * 16u);
+    uint4* d = reinterpret_cast<uint4*>(stage0 + b * uint32_t(kBinChunk));
+    for (uint32_t o = 0; o < np; o += 2048u)                 // <= 32 KB per bulk copy
+      tma_bulk_load(d + o, P.base16 + pa + o, min(2048u, np - o) * 16u, mbar + b);
+    const int64_t first = int64_t(2ull * pa) - int64_t(P.head);           // digit index of slot 0
+    s_par[4u * b] = s;
+    s_par[4u * b + 1u] = uint32_t(max(int64_t(P.off[s]) - first, int64_t(0)));
+    s_par[4u * b + 2u] = uint32_t(min(int64_t(P.off[s + 1]) - first, int64_t(2u * np)));
+  };
+  const uint32_t bpr = P.bins_per_row;
+  const uint32_t t_span = uint32_t(P.t_hi - P.t_lo);
+  // flush every partly filled buffer of sector s (padded with zero entries to a whole sector)
+  auto flush_all = [&](uint32_t s) {
+    uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
+    for (uint32_t bin = tid; bin < P.nb; bin += kBinThreads) {
+      const uint32_t n = cnt[bin];                            // < 8: fuller bins were flushed in phase B1
+      if (n) {
+        for (uint32_t x = n; x < 8u; ++x) buf[bin * 8u + x] = 0u;
+        const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
+        const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
+        const uint32_t row = bin / bpr, tb = bin - row * bpr, cap = r_cap[row];
+        const uint32_t base = atomicAdd(&counts[s * P.nb + bin], 8u);
+        if (base + 8u <= cap) {
+          uint32_t* d = seclist + r_off[row] + tb * cap + base;
+          st_v4(d, a);
+          st_v4(d + 4, c);
+        }
+        cnt[bin] = 0u;
+      }
     }
-    for (uint32_t i = tid; i < P.nb; i += kBinThreads) hist[i] = 0u;
-    // slots [slot_lo, slot_hi) of the chunk hold digits of sector s (slot j = digit first + j)
-    uint32_t slot_lo, slot_hi;
+    __syncthreads();
+  };
+
+  uint32_t s = 0, parbits = 0u;                            // bit b: wait parity of staging buffer b
+  if (k0 < k1) {
+    s = sector_of(k0, 0);
+    if (tid == 0) load(k0, s, 0);
+  }
+  __syncthreads();
+  for (uint32_t k = k0; k < k1; ++k) {
+    const uint32_t b = (k - k0) & 1u;
     {
-      const int64_t first = int64_t(2ull * pa) - int64_t(P.head);
-      slot_lo = uint32_t(max(int64_t(P.off[s]) - first, int64_t(0)));
-      slot_hi = uint32_t(min(int64_t(P.off[s + 1]) - first, int64_t(2u * np)));
+      const uint32_t s_new = s_par[4u * b];
+      if (s_new != s) {
+        flush_all(s);
+        s = s_new;
+      }
     }
+    if (tid == 0 && k + 1 < k1) load(k + 1, sector_of(k + 1, s), b ^ 1u);   // lands while this chunk is processed
+    const uint32_t slot_lo = s_par[4u * b + 1u], slot_hi = s_par[4u * b + 2u];
     const uint32_t cbase = s * P.nb;
     uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
-    __syncthreads();
-    mbar_wait(mbar, parity);
-    parity ^= 1u;
+    uint4* stage4 = reinterpret_cast<uint4*>(stage0 + b * uint32_t(kBinChunk));
+    uint32_t* nsecp = s_ctl + b;                             // second entries of this chunk
+    mbar_wait(mbar + b, (parbits >> b) & 1u);
+    parbits ^= 1u << b;
 
-    // ---- phase 1: quantise (D1), validate, rank inside the bin; overwrite the digit in place ----
-#pragma unroll 4
-    for (int i = 0; i < kBinPer; ++i) {
-      const uint32_t j = uint32_t(i) * kBinThreads + tid;
-      uint2 e = make_uint2(0u, kBinNone);
-      if (j >= slot_lo && j < slot_hi) {
-        const uint2 v = stage[j];
-        const uint32_t row = v.x & 0xFFu, pad = (v.x >> 8) & 0xFFu;
-        const int32_t time = int32_t(v.x >> 16);
-        const uint32_t q = quantise_q16(__uint_as_float(v.y));
-        if (q == 0u || time < P.t_lo || time >= P.t_hi || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
-          ++dropped;
-        } else {
-          const int32_t u = time - P.t_core_begin;
-          const int32_t tlo = max((u - kReach) >> kTileShift, 0);
-          const int32_t thi = min((u + kReach) >> kTileShift, tpr - 1);
-          if (tlo <= thi) {
-            const uint32_t bin = row * uint32_t(tpr) + uint32_t(tlo);
-            e.x = pack_digit(pad, uint32_t(u - (tlo << kTileShift) + kReach), q);
-            e.y = bin | (atomicAdd(&hist[bin], 1u) << 14);
-            if (thi != tlo) {                                 // also in the next tile's window
-              const uint32_t pk2 = e.x - (uint32_t(kTileT) << 8);
-              const uint32_t k2 = atomicAdd(&s_ovf[0], 1u);
-              if (k2 < uint32_t(kBinOvfCap)) {
-                ovf[k2] = make_uint2(pk2, (bin + 1u) | (atomicAdd(&hist[bin + 1u], 1u) << 14));
-              } else {                                        // overflow list full: direct global path
-                const uint32_t cap = r_cap[row];
-                const uint32_t slot = atomicAdd(&counts[cbase + bin + 1u], 1u);
-                if (slot < cap) seclist[r_off[row] + uint32_t(tlo + 1) * cap + slot] = pk2;
+    // rank an entry inside its bin; ranks 0..7 go to the bin's buffer
+    auto insert = [&](uint32_t bin, uint32_t pk) -> uint32_t {
+      const uint32_t r = atomicAdd(&cnt[bin], 1u);
+      if (r < 8u) buf[bin * 8u + r] = pk;
+      return r;
+    };
+    // ---- phase A: quantise (D1), validate, rank; overwrite the digit in place ----
+#pragma unroll
+    for (int i = 0; i < kBinPer / 2; ++i) {
+      const uint32_t pi = uint32_t(i) * kBinThreads + tid;
+      const uint4 v = stage4[pi];
+      uint32_t ex[2], ey[2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t w0 = h ? v.z : v.x, w1 = h ? v.w : v.y;
+        const uint32_t j = 2u * pi + uint32_t(h);
+        ex[h] = 0u;
+        ey[h] = kBinNone;
+        if (j - slot_lo < slot_hi - slot_lo) {
+          const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
+          const int32_t time = int32_t(w0 >> 16);
+          const uint32_t q = quantise_q16(__uint_as_float(w1));
+          if (q == 0u || uint32_t(time - P.t_lo) >= t_span || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
+            ++dropped;
+          } else {
+            const int32_t u = time - P.t_core_begin;
+            const int32_t tlo = max((u - kReach) >> kBinShift, 0);
+            const int32_t thi = min((u + kReach) >> kBinShift, int32_t(bpr) - 1);
+            if (tlo <= thi) {
+              const uint32_t bin = row * bpr + uint32_t(tlo);
+              const uint32_t pk = pack_digit(pad, uint32_t(u - (tlo << kBinShift) + kReach), q);
+              ex[h] = pk;
+              ey[h] = bin | (insert(bin, pk) << 12);
+              if (thi != tlo) {                               // also in the next bin's window
+                const uint32_t pk2 = pk - (uint32_t(kBinT) << 8);
+                const uint32_t k2 = atomicAdd(nsecp, 1u);
+                if (k2 < uint32_t(kBinSecCap)) {
+                  sec[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
+                } else {                                      // second-entry list full: reserve-8 direct path
+                  const uint32_t cap = r_cap[row];
+                  bin_append<8>(seclist, &counts[cbase + bin + 1u], r_off[row] + uint32_t(tlo + 1) * cap, cap, pk2);
+                }
               }
             }
           }
         }
       }
-      stage[j] = e;
+      stage4[pi] = make_uint4(ex[0], ey[0], ex[1], ey[1]);
     }
-    __syncthreads();                  // every entry is ranked, hist is complete
+    __syncthreads();                  // every entry is ranked; buffers and counts are complete
 
-    // ---- phase 2: one global reservation per non-empty bin, four in flight per thread ----
+    // ---- phase B1: bins holding a whole sector: reserve the whole sectors (one global atomic per
+    //      bin, up to four in flight per thread), store the buffered sector, keep the remainder ----
+    if (tid == 0) s_ctl[b ^ 1u] = 0u; // the other buffer's counter is idle until the next chunk's phase A
     for (uint32_t b0 = tid; b0 < P.nb; b0 += 4u * kBinThreads) {
-      uint32_t c[4], g[4];
+      uint32_t n[4], g[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const uint32_t b = b0 + uint32_t(u) * kBinThreads;
-        c[u] = b < P.nb ? hist[b] : 0u;
+      for (int x = 0; x < 4; ++x) {
+        const uint32_t bin = b0 + uint32_t(x) * kBinThreads;
+        n[x] = bin < P.nb ? cnt[bin] : 0u;
       }
 #pragma unroll
-      for (int u = 0; u < 4; ++u)
-        g[u] = c[u] ? atomicAdd(&counts[cbase + b0 + uint32_t(u) * kBinThreads], c[u]) : 0u;
+      for (int x = 0; x < 4; ++x)
+        g[x] = n[x] >= 8u ? atomicAdd(&counts[cbase + b0 + uint32_t(x) * kBinThreads], n[x] & ~7u) : 0u;
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        if (c[u]) {
-          const uint32_t b = b0 + uint32_t(u) * kBinThreads;
-          const uint32_t row = b / uint32_t(tpr), tt = b - row * uint32_t(tpr);
-          const uint32_t cap = r_cap[row];
-          hist[b] = (g[u] + c[u] <= cap) ? r_off[row] + tt * cap + g[u] : kBinFull;
+      for (int x = 0; x < 4; ++x) {
+        if (n[x] >= 8u) {
+          const uint32_t bin = b0 + uint32_t(x) * kBinThreads;
+          const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
+          const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
+          const uint32_t row = bin / bpr, tb = bin - row * bpr, cap = r_cap[row];
+          uint32_t d = kBinFull;
+          if (g[x] + (n[x] & ~7u) <= cap) {
+            d = r_off[row] + tb * cap + g[x];
+            st_v4(seclist + d, a);
+            st_v4(seclist + d + 4, c);
+          }
+          dst[bin] = d;
+          nfull[bin] = uint16_t(n[x] >> 3);
+          cnt[bin] = n[x] & 7u;       // entries ranked >= 8 * nfull move to the buffer's front in phase B2
         }
       }
     }
     __syncthreads();
 
-    // ---- phase 3: store the packed digits at reservation + rank ----
-#pragma unroll 4
-    for (int i = 0; i < kBinPer; ++i) {
-      const uint2 e = stage[uint32_t(i) * kBinThreads + tid];
-      if (e.y != kBinNone) {
-        const uint32_t d = hist[e.y & 0x3FFFu];
-        if (d != kBinFull) seclist[d + (e.y >> 14)] = e.x;
+    // ---- phase B2: entries ranked >= 8: into the reserved sectors, or back into the (now empty) buffer ----
+    auto place = [&](uint32_t pk, uint32_t y) {
+      const uint32_t bin = y & 0xFFFu, r = y >> 12;
+      const uint32_t nf8 = uint32_t(nfull[bin]) << 3;
+      if (r >= nf8) {
+        buf[bin * 8u + (r - nf8)] = pk;
+      } else {
+        const uint32_t d = dst[bin];
+        if (d != kBinFull) seclist[d + r] = pk;
       }
+    };
+#pragma unroll
+    for (int i = 0; i < kBinPer / 2; ++i) {
+      const uint4 v = stage4[uint32_t(i) * kBinThreads + tid];
+      if (v.y != kBinNone && (v.y >> 12) >= 8u) place(v.x, v.y);
+      if (v.w != kBinNone && (v.w >> 12) >= 8u) place(v.z, v.w);
     }
     {
-      const uint32_t novf = min(s_ovf[0], uint32_t(kBinOvfCap));
-      for (uint32_t i = tid; i < novf; i += kBinThreads) {
-        const uint2 e = ovf[i];
-        const uint32_t d = hist[e.y & 0x3FFFu];
-        if (d != kBinFull) seclist[d + (e.y >> 14)] = e.x;
+      const uint32_t nsec = min(*nsecp, uint32_t(kBinSecCap));
+      for (uint32_t i = tid; i < nsec; i += kBinThreads) {
+        const uint2 e = sec[i];
+        if ((e.y >> 12) >= 8u) place(e.x, e.y);
       }
     }
-    __syncthreads();                  // stage, hist and the overflow list are reused by the next chunk
+    __syncthreads();                  // buffers, staging area and lists are reused by the next chunk
   }
+  if (k0 < k1) flush_all(s);
   dropped = __reduce_add_sync(0xffffffffu, dropped);
   if ((tid & 31u) == 0u && dropped) atomicAdd(&status->n_dropped, (unsigned long long)dropped);
 }
@@ -740,12 +840,13 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
   const uint32_t sub = lane & 3u;                                      // build phase: lane frame R_sub
   const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
   // address and (clamped) length of a tile's digit list
+  // (a tile is one half of a kBinT-wide bin: both halves stage the same list)
   auto tile_list = [&](uint32_t t, const uint32_t*& src) -> uint32_t {
-    const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
+    const uint32_t sr = t / P.tiles_per_row, tb = (t - sr * P.tiles_per_row) / uint32_t(kTilesPerBin);
     const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
     const uint32_t cap = P.rows[row].cap;
-    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tt) * cap;
-    return min(P.counts[t], cap);
+    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tb) * cap;
+    return min(P.counts[sr * P.bins_per_row + tb], cap);
   };
   // stage digits [c0, c0+m) of a list in lbuf (one thread)
   auto issue = [&](const uint32_t* src, uint32_t c0, uint32_t m) {
@@ -778,6 +879,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
     const uint32_t W = ri.W, wpr = W >> 1;
+    const uint32_t tl_off = (tt % uint32_t(kTilesPerBin)) * uint32_t(kTileT);   // this tile's first row in the bin window
     uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
     uint32_t* bm = reinterpret_cast<uint32_t*>(mapraw + uint32_t(kBoxH) * W * 2u);   // W % 8 == 0: 16-byte aligned
     const uint32_t* src = nullptr;
@@ -802,7 +904,8 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       parity ^= 1u;
       for (uint32_t i = tid; i < m; i += kWorkThreads) {
         const uint32_t d = lbuf[i];
-        map[dig_tl(d) * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));
+        const uint32_t tl = dig_tl(d) - tl_off;                           // row in this tile's window, if < kBoxH
+        if (d != 0u && tl < uint32_t(kBoxH)) map[tl * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
       }
     }
     bar_sync_named(kBarWork, kWorkThreads);
@@ -820,7 +923,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
         }
         for (uint32_t i = tid; i < m; i += kWorkThreads) {
           const uint32_t d = lbuf[i];
-          const uint32_t q16 = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
+          const uint32_t q16 = dig_q(d), tl = dig_tl(d) - tl_off, pad = dig_pad(d);
           if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
             atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
         }
