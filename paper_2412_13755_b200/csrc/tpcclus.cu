@@ -198,7 +198,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = kDigCap * 4 + c->map_bytes_max + 2 * kListCap * 32 + 16 + 16 + 16 * 4 + 2 * 4 * 4 + kListCap * 4 +
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + 16 + 32 * 4 + 2 * 4 * 4 + kListCap * 4 +
                   (kTileT + 4) * 4 + kNbrTabWords * 4 + 12 * 4 + 128;
 
   int rc;
@@ -352,7 +352,6 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     tp.n_sectors = g.n_sectors;
     tp.n_rows = g.n_rows;
     tp.tiles_per_row = tiles_per_row;
-    tp.bins_per_row = bins_per_row;
     tp.n_tiles = n_tiles;
     tp.t_core_begin = int32_t(b);
     tp.t_core_end = int32_t(e);

@@ -25,19 +25,17 @@
 
 namespace tpcclus {
 
-constexpr int      kThreads      = 256;   // CTA size of k_tile
-constexpr int      kWorkThreads  = 224;   // warps 0..6 run S1..S5 on the tiles; warp 7 commits (look-back + copy-out)
-constexpr int      kTileT        = 128;   // core time bins per tile
+constexpr int      kThreads      = 512;   // CTA size of k_tile (two CTAs per SM)
+constexpr int      kWorkThreads  = 480;   // warps 0..14 run S1..S5 on the tiles; warp 15 commits (look-back + copy-out)
+constexpr int      kTileT        = 256;   // core time bins per tile (= one digit bin of k_bin)
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
 constexpr int      kBinT         = 256;   // core time bins per digit bin (= two tiles: k_tile filters by half)
 constexpr int      kBinShift     = 8;
 constexpr int      kBinBoxH      = kBinT + 2 * kReach;    // time rows a bin's window spans (266)
-static_assert((1 << kBinShift) == kBinT && kBinT % kTileT == 0, "bins are whole tiles");
-constexpr int      kTilesPerBin  = kBinT / kTileT;
+static_assert((1 << kBinShift) == kBinT && kBinT == kTileT, "a digit bin is one tile");
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
-constexpr int      kListCap      = 160;   // peaks per hand-over item (capacity of one staging buffer)
-constexpr int      kDigCap       = 4096;  // digits staged per TMA bulk copy (16 KB)
+constexpr int      kListCap      = 136;   // peaks per hand-over item (capacity of one staging buffer; > 128 = most peaks of a row)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 
@@ -86,7 +84,6 @@ struct TileParams {
   uint64_t           sec_list_elems;
   uint32_t n_sectors, n_rows;
   uint32_t tiles_per_row;              // ceil((e-b)/kTileT)
-  uint32_t bins_per_row;               // ceil((e-b)/kBinT)
   uint32_t n_tiles;
   int32_t  t_core_begin, t_core_end;   // [b,e)
   uint32_t tf_time_bins;
@@ -787,16 +784,14 @@ __device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-__global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ TileParams P) {
+__global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ TileParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
   uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
-  uint32_t* lbuf = reinterpret_cast<uint32_t*>(sp);         sp += kDigCap * 4;   // TMA bulk destination
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);         sp += 16;
   uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // [0] tile, [1] digits (next tile)
-  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 16 * 4;        // [1..7] warp totals, [12] next peak group
+  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 32 * 4;        // [1..15] warp totals, [20] next peak group
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
   uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
   uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
@@ -805,10 +800,6 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t bmw = P.bm_words;
-  if (tid == 0) {
-    mbar_init(mbar, 1);
-    fence_mbar_init();
-  }
   for (uint32_t i = tid; i < uint32_t(kNbrTabWords); i += kThreads) nbr_tab[i] = nbr_tab_entry(i);
   if (tid < 9u) wtab[tid] = kShareL / (tid + 1u);
   __syncthreads();
@@ -839,39 +830,22 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
   // ================= worker warps =================
   const uint32_t sub = lane & 3u;                                      // build phase: lane frame R_sub
   const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
-  // address and (clamped) length of a tile's digit list
-  // (a tile is one half of a kBinT-wide bin: both halves stage the same list)
+  // address and (clamped) length of a tile's digit list (tile = bin: kTileT == kBinT)
   auto tile_list = [&](uint32_t t, const uint32_t*& src) -> uint32_t {
-    const uint32_t sr = t / P.tiles_per_row, tb = (t - sr * P.tiles_per_row) / uint32_t(kTilesPerBin);
+    const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
     const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
     const uint32_t cap = P.rows[row].cap;
-    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tb) * cap;
-    return min(P.counts[sr * P.bins_per_row + tb], cap);
+    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tt) * cap;
+    return min(P.counts[t], cap);
   };
-  // stage digits [c0, c0+m) of a list in lbuf (one thread)
-  auto issue = [&](const uint32_t* src, uint32_t c0, uint32_t m) {
-    const uint32_t bytes = ((m + 3u) & ~3u) * 4u;              // bins are padded to a multiple of 4 digits
-    mbar_arrive_expect_tx(mbar, bytes);
-    tma_bulk_load(lbuf, src + c0, bytes, mbar);
-  };
-  // take the next tile in ticket order and start staging its list (one thread)
-  auto fetch = [&]() {
-    const uint32_t t = atomicAdd(&P.status->ticket, 1u);
-    uint32_t n = 0;
-    if (t < P.n_tiles) {
-      const uint32_t* src;
-      n = tile_list(t, src);
-      if (n) issue(src, 0, min(n, uint32_t(kDigCap)));
-    }
-    s_next[0] = t;
-    s_next[1] = n;
-  };
+  // take the next tile in ticket order (one thread)
+  auto fetch = [&]() { s_next[0] = atomicAdd(&P.status->ticket, 1u); };
   if (tid == 0) fetch();
   bar_sync_named(kBarWork, kWorkThreads);
 
-  uint32_t parity = 0, q = 0;                                          // q: hand-over items issued so far
+  uint32_t q = 0;                                                      // hand-over items issued so far
   for (;;) {
-    const uint32_t t = s_next[0], n = s_next[1];
+    const uint32_t t = s_next[0];
     if (t >= P.n_tiles) break;
     const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
     const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
@@ -879,58 +853,64 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
     const uint32_t W = ri.W, wpr = W >> 1;
-    const uint32_t tl_off = (tt % uint32_t(kTilesPerBin)) * uint32_t(kTileT);   // this tile's first row in the bin window
     uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
     uint32_t* bm = reinterpret_cast<uint32_t*>(mapraw + uint32_t(kBoxH) * W * 2u);   // W % 8 == 0: 16-byte aligned
-    const uint32_t* src = nullptr;
-    if (n > uint32_t(kDigCap)) tile_list(t, src);                        // only big tiles stage more than once
+    const uint32_t* src;
+    const uint32_t n = tile_list(t, src);                                // a multiple of 8; 0 entries are padding
+    const uint4* src4 = reinterpret_cast<const uint4*>(src);
+    const uint32_t n4 = n >> 2;
 
-    // ---- D2: zero the tile's charge map and flag bitmap (the list is landing meanwhile) ----
+    // ---- D2: zero the tile's charge map and flag bitmap ----
     {
       const uint32_t nz = (uint32_t(kBoxH) * W * 2u + uint32_t(kBoxH) * bmw * 4u + 15u) >> 4;
       uint4* z = reinterpret_cast<uint4*>(mapraw);
       for (uint32_t i = tid; i < nz; i += kWorkThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     bar_sync_named(kBarWork, kWorkThreads);
+    if (tid == 0) fetch();                    // next tile's ticket (s_next is read again after later barriers)
 
-    // ---- S1: scatter the staged digits into the map ----
-    for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
-      const uint32_t m = min(n - c0, uint32_t(kDigCap));
-      if (c0) {
-        bar_sync_named(kBarWork, kWorkThreads);
-        if (tid == 0) issue(src, c0, m);
+    // ---- S1: scatter the list into the map (16-byte streaming loads, two in flight per thread) ----
+    {
+      auto put = [&](uint32_t d) {
+        if (d) map[dig_tl(d) * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
+      };
+      uint32_t i = tid;
+      for (; i + kWorkThreads < n4; i += 2 * kWorkThreads) {
+        const uint4 a = __ldg(src4 + i), c = __ldg(src4 + i + kWorkThreads);
+        put(a.x); put(a.y); put(a.z); put(a.w);
+        put(c.x); put(c.y); put(c.z); put(c.w);
       }
-      mbar_wait(mbar, parity);
-      parity ^= 1u;
-      for (uint32_t i = tid; i < m; i += kWorkThreads) {
-        const uint32_t d = lbuf[i];
-        const uint32_t tl = dig_tl(d) - tl_off;                           // row in this tile's window, if < kBoxH
-        if (d != 0u && tl < uint32_t(kBoxH)) map[tl * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
+      if (i < n4) {
+        const uint4 a = __ldg(src4 + i);
+        put(a.x); put(a.y); put(a.z); put(a.w);
       }
     }
     bar_sync_named(kBarWork, kWorkThreads);
 
-    // ---- S2: D4 peak flags for map rows 1..136, digit-driven ----
+    // ---- S2: D4 peak flags for map rows 1..kBoxH-2, digit-driven (the list is in L1/L2 now) ----
     {
       const uint32_t* map32 = reinterpret_cast<const uint32_t*>(map);
-      for (uint32_t c0 = 0; c0 < n; c0 += kDigCap) {
-        const uint32_t m = min(n - c0, uint32_t(kDigCap));
-        if (n > uint32_t(kDigCap)) {                                     // re-stage (the first pass overwrote lbuf)
-          bar_sync_named(kBarWork, kWorkThreads);
-          if (tid == 0) issue(src, c0, m);
-          mbar_wait(mbar, parity);
-          parity ^= 1u;
-        }
-        for (uint32_t i = tid; i < m; i += kWorkThreads) {
-          const uint32_t d = lbuf[i];
-          const uint32_t q16 = dig_q(d), tl = dig_tl(d) - tl_off, pad = dig_pad(d);
-          if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
-            atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
-        }
+      auto test = [&](uint32_t d) {
+        const uint32_t q16 = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
+        if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
+          atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
+      };
+      for (uint32_t i = tid; i < n4; i += kWorkThreads) {
+        const uint4 a = __ldg(src4 + i);
+        test(a.x); test(a.y); test(a.z); test(a.w);
       }
     }
-    bar_sync_named(kBarWork, kWorkThreads);   // flags complete; lbuf is free
-    if (tid == 0) fetch();                    // next tile's ticket; its list lands during count + build
+    // pull the next tile's list towards L2 while this tile is counted and built
+    {
+      const uint32_t tn = s_next[0];
+      if (tn < P.n_tiles) {
+        const uint32_t* nsrc;
+        const uint32_t nn = tile_list(tn, nsrc);
+        for (uint32_t i = tid * 32u; i < nn; i += kWorkThreads * 32u)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(nsrc + i));
+      }
+    }
+    bar_sync_named(kBarWork, kWorkThreads);   // flags complete
 
     // ---- S6 (in-tile part): ordered count of the core rows, block scan ----
     uint32_t cnt = 0;
@@ -978,7 +958,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
           }
         }
       }
-      if (tid == 0) s_misc[12] = 0u;
+      if (tid == 0) s_misc[20] = 0u;
       bar_sync_named(kBarWork, kWorkThreads);
       // peaks of this item: all that are left, or the longest prefix of whole rows that fits
       uint32_t npass = total - done;
@@ -1000,7 +980,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       uint4* stg = stage + b * (2u * kListCap);
       for (;;) {
         uint32_t g = 0;
-        if (lane == 0) g = atomicAdd(&s_misc[12], 1u);
+        if (lane == 0) g = atomicAdd(&s_misc[20], 1u);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g * 8u >= npass) break;
         const uint32_t i = g * 8u + (lane >> 2);
@@ -1013,7 +993,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_tile(const __grid_constant__ Ti
       bar_arrive_named(kBarFull + int(b), kThreads);
       ++q;
       done += npass;
-      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // plist and s_misc[12] are reused
+      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // plist and s_misc[20] are reused
     } while (done < total);
     bar_sync_named(kBarWork, kWorkThreads);   // map, bitmap and s_next are stable until here
   }
