@@ -856,7 +856,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
     uint32_t* bm = reinterpret_cast<uint32_t*>(mapraw + uint32_t(kBoxH) * W * 2u);   // W % 8 == 0: 16-byte aligned
     const uint32_t* src;
-    const uint32_t n = tile_list(t, src);                                // a multiple of 8; 0 entries are padding
+    const uint32_t n = tile_list(t, src);                                // k_bin: a multiple of 8; 0 entries are padding
     const uint4* src4 = reinterpret_cast<const uint4*>(src);
     const uint32_t n4 = n >> 2;
 
@@ -884,6 +884,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         const uint4 a = __ldg(src4 + i);
         put(a.x); put(a.y); put(a.z); put(a.w);
       }
+      if (tid < (n & 3u)) put(__ldg(src + 4u * n4 + tid));               // k_bin_direct lists: any length
     }
     bar_sync_named(kBarWork, kWorkThreads);
 
@@ -899,6 +900,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         const uint4 a = __ldg(src4 + i);
         test(a.x); test(a.y); test(a.z); test(a.w);
       }
+      if (tid < (n & 3u)) test(__ldg(src + 4u * n4 + tid));
     }
     // pull the next tile's list towards L2 while this tile is counted and built
     {

@@ -243,3 +243,78 @@ def test_host_api_single_and_tf():
         assert T.tpcclus_launch_count(ctx) == 4 * 4 and T.tpcclus_device_bytes(ctx) > 0
     finally:
         T.tpcclus_destroy(ctx)
+
+
+def _sorted_within_sectors(dn, offs, keys):
+    out = dn.copy()
+    for s in range(len(offs) - 1):
+        a, b = int(offs[s]), int(offs[s + 1])
+        seg = dn[a:b]
+        out[a:b] = seg[np.lexsort(tuple(seg[k] for k in reversed(keys)))]
+    return out
+
+
+@pytest.mark.parametrize("order", ["row_time_pad", "time_row_pad", "reverse"])
+def test_sorted_digit_orders(order):
+    """Digit order inside a sector slice is arbitrary.  Sorted input is the worst
+    case for the write-combining binning kernel: a whole chunk of consecutive digits falls into one
+    or two bins (ranks far beyond a buffer, several sectors reserved at once, time-major order puts
+    every digit of a chunk next to a bin seam).  Output must be byte-identical to the shuffled run
+    and to the oracle."""
+    cfg = gen.config("c2mini", tf_time_bins=600, core_bins=600)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    if order == "row_time_pad":
+        sn = _sorted_within_sectors(dn, offs, ["row", "time", "pad"])
+    elif order == "time_row_pad":
+        sn = _sorted_within_sectors(dn, offs, ["time", "row", "pad"])
+    else:
+        sn = _sorted_within_sectors(dn, offs, ["row", "time", "pad"])
+        for s in range(len(offs) - 1):
+            a, b = int(offs[s]), int(offs[s + 1])
+            sn[a:b] = sn[a:b][::-1]
+    kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    shuffled, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
+    got, st = gpu_clusters(sn, offs, cfg.npads_array(), **kw)
+    ref, ost = oracle.run(dn, offs, cfg.npads_array(), **kw)
+    assert len(ref) > 1e4 and st["n_digits_dropped"] == ost["n_digits_dropped"] == 0
+    assert got.tobytes() == shuffled.tobytes()
+    assert_clusters_match(got, ref, order)
+
+
+def test_unaligned_digit_buffer_and_sector_seams():
+    """The digit buffer only has to be 8-byte aligned; sector slices may start on odd digits, so the
+    16-byte pairs at slice seams hold digits of two sectors (k_bin's slot_lo / slot_hi logic)."""
+    import torch
+
+    cfg = gen.config("c2mini", tf_time_bins=300, core_bins=300)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    # drop one digit of sector 0 so that sector 1 starts on an odd index; then shift the buffer by 8 bytes
+    dn2 = np.concatenate([dn[:1], dn[2:]])
+    offs2 = np.array(offs, dtype=np.uint64).copy()
+    offs2[1:] -= 1
+    ref, _ = oracle.run(dn2, offs2, cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    for shift in (0, 1):
+        raw = torch.zeros((len(dn2) + shift + 1, 8), dtype=torch.uint8, device="cuda")
+        view = raw[shift: shift + len(dn2)]
+        view.copy_(to_device_digits(dn2))
+        assert view.data_ptr() % 8 == 0 and (view.data_ptr() - raw.data_ptr()) == 8 * shift
+        with GpuClusterizer(cfg.npads_array(), n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins,
+                            max_digits=len(dn2)) as g:
+            got, st = g.run(view, offs2, 0, cfg.tf_time_bins)
+        assert st["n_digits_dropped"] == 0
+        assert got.tobytes() == ref.tobytes(), shift
+
+
+def test_direct_binning_fallback_matches(monkeypatch):
+    """k_bin_direct (taken when a geometry's bins do not fit the write-combining kernel's shared
+    memory; forced here with TPCCLUS_BIN_DIRECT=1) gives the same bytes."""
+    cfg = gen.config("c4mini", tf_time_bins=300, core_bins=300)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    a, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
+    monkeypatch.setenv("TPCCLUS_BIN_DIRECT", "1")
+    b, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
+    assert len(a) > 1e4 and a.tobytes() == b.tobytes()
