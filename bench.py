@@ -299,11 +299,11 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (algorithmic bytes per launch / mean launch time) ----
     peak, peak_src = measured_peak_gbs()
     nfr = len(tf)
-    # digits appended to the tile lists: every digit once, plus once more when it lies within
-    # 5 bins of a 128-bin tile seam (10/128 of the core bins)
-    dup = 1.0 + 10.0 / 128.0
+    # entries appended to the bin lists: every digit once, plus once more when it lies within
+    # 5 bins of a 256-bin seam (10/256 of the core bins)
+    dup = 1.0 + 10.0 / 256.0
     alg = {   # bytes per launch, DESIGN.md §6
-        "k_init": 4.0 * cfg.n_sectors * cfg.n_rows * ((cfg.core_bins + 127) // 128),   # one counter per tile
+        "k_init": 4.0 * cfg.n_sectors * cfg.n_rows * ((cfg.core_bins + 255) // 256),   # one counter per bin
         "k_bin": (8.0 + 4.0 * dup) * n_dig / nfr,                 # read 8 B/digit, append 4 B per list entry
         "k_tile": (4.0 * dup * n_dig + 32.0 * n_cl) / nfr,        # read every list entry once, write every record
         "k_finish": 64.0 * n_cl / nfr,                            # integer moments -> float fields, in place
