@@ -181,10 +181,9 @@ __device__ __forceinline__ uint32_t dig_tl(uint32_t d) { return (d >> 8) & 0x1FF
 __device__ __forceinline__ uint32_t dig_q(uint32_t d) { return d >> 17; }
 
 __device__ __forceinline__ uint32_t quantise_q16(float charge) {
-  // D1: q16 = clamp(rint(charge*16), 0, 16368); rint = round-half-even (cvt.rni); NaN -> 0
-  const float x = rintf(charge * 16.0f);
-  if (!(x > 0.0f)) return 0u;                    // also catches NaN
-  return x >= float(kQClamp) ? kQClamp : uint32_t(x);
+  // D1: q16 = clamp(rint(charge*16), 0, 16368).  cvt.rni.u32.f32 rounds half-even and saturates:
+  // negative and NaN -> 0, huge -> 0xFFFFFFFF
+  return min(__float2uint_rn(charge * 16.0f), kQClamp);
 }
 
 // append one packed digit to a bin, reserving R slots (R = 1: k_bin_direct; R = 8: the odd
@@ -327,7 +326,12 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   const uint32_t tid = threadIdx.x;
   for (uint32_t i = tid; i < 256u; i += kBinThreads) {
     const bool in = i < P.n_rows;
-    r_npads[i] = in ? rows[i].npads : 0u;
+    if (i < 64u) {                                            // npads - 1 as bytes, four rows per word
+      uint32_t w = 0;
+      for (uint32_t k = 0; k < 4u; ++k)
+        if (4u * i + k < P.n_rows) w |= (uint32_t(rows[4u * i + k].npads) - 1u) << (8u * k);
+      r_npads[i] = w;
+    }
     r_off[i] = in ? rows[i].list_off : 0u;
     r_cap[i] = in ? rows[i].cap : 0u;
   }
@@ -416,6 +420,15 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     if (tid == 0) load(k0, s, 0);
   }
   __syncthreads();
+  // phase B1 visits bins tid, tid + 1024, ...: their list offsets and capacities never change
+  uint32_t b_off[4], b_cap[4];
+#pragma unroll
+  for (int x = 0; x < 4; ++x) {
+    const uint32_t bin = tid + uint32_t(x) * kBinThreads;
+    const uint32_t row = min(bin / bpr, 255u), tb = bin - (bin / bpr) * bpr;
+    b_cap[x] = r_cap[row];
+    b_off[x] = r_off[row] + tb * b_cap[x];
+  }
   for (uint32_t k = k0; k < k1; ++k) {
     const uint32_t b = (k - k0) & 1u;
     {
@@ -427,6 +440,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     }
     if (tid == 0 && k + 1 < k1) load(k + 1, sector_of(k + 1, s), b ^ 1u);   // lands while this chunk is processed
     const uint32_t slot_lo = s_par[4u * b + 1u], slot_hi = s_par[4u * b + 2u];
+    const bool full_chunk = slot_lo == 0u && slot_hi == uint32_t(kBinChunk);   // no sector seam inside: no per-digit check
     const uint32_t cbase = s * P.nb;
     uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
     uint4* stage4 = reinterpret_cast<uint4*>(stage0 + b * uint32_t(kBinChunk));
@@ -440,23 +454,24 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
       if (r < 8u) buf[bin * 8u + r] = pk;
       return r;
     };
-    // ---- phase A: quantise (D1), validate, rank; overwrite the digit in place ----
+    // ---- phase A: quantise (D1), validate, rank.  An entry ranked >= 8 (its bin's buffer is full)
+    //      overwrites its digit in the staging area and is remembered in `pend` for phase B2 ----
+    uint32_t pend = 0;
+    uint2* stage2 = reinterpret_cast<uint2*>(stage4);
 #pragma unroll
     for (int i = 0; i < kBinPer / 2; ++i) {
       const uint32_t pi = uint32_t(i) * kBinThreads + tid;
       const uint4 v = stage4[pi];
-      uint32_t ex[2], ey[2];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const uint32_t w0 = h ? v.z : v.x, w1 = h ? v.w : v.y;
         const uint32_t j = 2u * pi + uint32_t(h);
-        ex[h] = 0u;
-        ey[h] = kBinNone;
-        if (j - slot_lo < slot_hi - slot_lo) {
+        if (full_chunk || j - slot_lo < slot_hi - slot_lo) {
           const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
           const int32_t time = int32_t(w0 >> 16);
           const uint32_t q = quantise_q16(__uint_as_float(w1));
-          if (q == 0u || uint32_t(time - P.t_lo) >= t_span || pad >= r_npads[row]) {   // r_npads = 0 past n_rows
+          const uint32_t last_pad = (r_npads[row >> 2] >> (8u * (row & 3u))) & 0xFFu;   // npads - 1
+          if (q == 0u || uint32_t(time - P.t_lo) >= t_span || pad > last_pad || row >= P.n_rows) {
             ++dropped;
           } else {
             const int32_t u = time - P.t_core_begin;
@@ -465,8 +480,11 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
             if (tlo <= thi) {
               const uint32_t bin = row * bpr + uint32_t(tlo);
               const uint32_t pk = pack_digit(pad, uint32_t(u - (tlo << kBinShift) + kReach), q);
-              ex[h] = pk;
-              ey[h] = bin | (insert(bin, pk) << 12);
+              const uint32_t r = insert(bin, pk);
+              if (r >= 8u) {
+                stage2[j] = make_uint2(pk, bin | (r << 12));
+                pend |= 1u << (2 * i + h);
+              }
               if (thi != tlo) {                               // also in the next bin's window
                 const uint32_t pk2 = pk - (uint32_t(kBinT) << 8);
                 const uint32_t k2 = atomicAdd(nsecp, 1u);
@@ -481,33 +499,31 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
           }
         }
       }
-      stage4[pi] = make_uint4(ex[0], ey[0], ex[1], ey[1]);
     }
     __syncthreads();                  // every entry is ranked; buffers and counts are complete
 
     // ---- phase B1: bins holding a whole sector: reserve the whole sectors (one global atomic per
     //      bin, up to four in flight per thread), store the buffered sector, keep the remainder ----
     if (tid == 0) s_ctl[b ^ 1u] = 0u; // the other buffer's counter is idle until the next chunk's phase A
-    for (uint32_t b0 = tid; b0 < P.nb; b0 += 4u * kBinThreads) {
+    {                                 // P.nb <= kBinMaxNb = 4 * kBinThreads
       uint32_t n[4], g[4];
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
-        const uint32_t bin = b0 + uint32_t(x) * kBinThreads;
+        const uint32_t bin = tid + uint32_t(x) * kBinThreads;
         n[x] = bin < P.nb ? cnt[bin] : 0u;
       }
 #pragma unroll
       for (int x = 0; x < 4; ++x)
-        g[x] = n[x] >= 8u ? atomicAdd(&counts[cbase + b0 + uint32_t(x) * kBinThreads], n[x] & ~7u) : 0u;
+        g[x] = n[x] >= 8u ? atomicAdd(&counts[cbase + tid + uint32_t(x) * kBinThreads], n[x] & ~7u) : 0u;
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
         if (n[x] >= 8u) {
-          const uint32_t bin = b0 + uint32_t(x) * kBinThreads;
+          const uint32_t bin = tid + uint32_t(x) * kBinThreads;
           const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
           const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
-          const uint32_t row = bin / bpr, tb = bin - row * bpr, cap = r_cap[row];
           uint32_t d = kBinFull;
-          if (g[x] + (n[x] & ~7u) <= cap) {
-            d = r_off[row] + tb * cap + g[x];
+          if (g[x] + (n[x] & ~7u) <= b_cap[x]) {
+            d = b_off[x] + g[x];
             st_v4(seclist + d, a);
             st_v4(seclist + d + 4, c);
           }
@@ -530,11 +546,11 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         if (d != kBinFull) seclist[d + r] = pk;
       }
     };
-#pragma unroll
-    for (int i = 0; i < kBinPer / 2; ++i) {
-      const uint4 v = stage4[uint32_t(i) * kBinThreads + tid];
-      if (v.y != kBinNone && (v.y >> 12) >= 8u) place(v.x, v.y);
-      if (v.w != kBinNone && (v.w >> 12) >= 8u) place(v.z, v.w);
+    while (pend) {                    // most lanes have none: the loop runs as long as some lane has one
+      const uint32_t e = __ffs(pend) - 1;
+      pend &= pend - 1;
+      const uint2 v = stage2[2u * ((e >> 1) * kBinThreads + tid) + (e & 1u)];
+      place(v.x, v.y);
     }
     {
       const uint32_t nsec = min(*nsecp, uint32_t(kBinSecCap));
