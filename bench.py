@@ -306,7 +306,6 @@ def run_ours(args):
         "k_init": 4.0 * cfg.n_sectors * cfg.n_rows * ((cfg.core_bins + 255) // 256),   # one counter per bin
         "k_bin": (8.0 + 4.0 * dup) * n_dig / nfr,                 # read 8 B/digit, append 4 B per list entry
         "k_tile": (4.0 * dup * n_dig + 32.0 * n_cl) / nfr,        # read every list entry once, write every record
-        "k_finish": 64.0 * n_cl / nfr,                            # integer moments -> float fields, in place
     }
     kern = {}
     for k, ms_sum in prof.items():

@@ -174,10 +174,9 @@ int tpcclus_run_tf_host(tpcclus_ctx* ctx, const tpcclus_fragment* frags, uint32_
                         tpcclus_run_stats* stats /* HOST [n_frags] */);
 
 /* Per-kernel device timing (for the roofline figures of bench.py): while on, every run is
- * bracketed with CUDA events on ITS stream around k_init (S0), k_bin (S1 routing), k_tile
- * (S1 fill .. S7) and k_finish (S5, D8 float fields); tpcclus_result adds the elapsed times
- * up.  set_profiling(1) resets the sums. */
-#define TPCCLUS_N_KERNELS 4
+ * bracketed with CUDA events on ITS stream around k_init (S0), k_bin (S1 routing) and k_tile
+ * (S1 fill .. S7); tpcclus_result adds the elapsed times up.  set_profiling(1) resets the sums. */
+#define TPCCLUS_N_KERNELS 3
 int tpcclus_set_profiling(tpcclus_ctx* ctx, int on);
 int tpcclus_get_profile(const tpcclus_ctx* ctx, double kernel_ms[TPCCLUS_N_KERNELS] /* HOST out */, uint64_t* n_runs /* HOST out */);
 

@@ -192,13 +192,13 @@ def tpcclus_set_profiling(ctx, on: bool) -> None:
 
 
 def tpcclus_get_profile(ctx):
-    """-> ({"k_init": ms, "k_bin": ms, "k_tile": ms, "k_finish": ms} summed over runs, n_runs)."""
-    ms = (ctypes.c_double * 4)()
+    """-> ({"k_init": ms, "k_bin": ms, "k_tile": ms} summed over runs, n_runs)."""
+    ms = (ctypes.c_double * 3)()
     n = ctypes.c_uint64()
     rc = lib().tpcclus_get_profile(ctx, ms, ctypes.byref(n))
     if rc != TPCCLUS_OK:
         raise TpcclusError(rc, "tpcclus_get_profile")
-    return dict(k_init=ms[0], k_bin=ms[1], k_tile=ms[2], k_finish=ms[3]), int(n.value)
+    return dict(k_init=ms[0], k_bin=ms[1], k_tile=ms[2]), int(n.value)
 
 
 def tpcclus_launch_count(ctx) -> int:

@@ -50,7 +50,7 @@ struct tpcclus_ctx {
   struct Pending { uint64_t n, cap; };
   Pending pending[kRing];
   cudaEvent_t ev_done[kRing] = {};
-  cudaEvent_t ev_prof[kRing][TPCCLUS_N_KERNELS + 1] = {};   // around k_init / k_bin / k_tile / k_finish when profiling
+  cudaEvent_t ev_prof[kRing][TPCCLUS_N_KERNELS + 1] = {};   // around k_init / k_bin / k_tile when profiling
   bool slot_profiled[kRing] = {};
   uint64_t head = 0, tail = 0;          // runs reported / runs enqueued
   cudaStream_t last_stream = nullptr;
@@ -366,15 +366,6 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     debug_check(st, "k_tile");
   }
   if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][3], st));
-  // S5 finish (D8): exact integer moments -> float32 fields, in place
-  if (cap) {
-    const uint64_t want = (std::min<uint64_t>(cap, g.max_clusters ? g.max_clusters : cap) + 255) / 256;
-    const uint32_t blocks = uint32_t(std::min<uint64_t>(std::max<uint64_t>(want, 1), uint64_t(c->n_sm) * 8));
-    k_finish<<<blocks, 256, 0, st>>>(d_out, cap, c->d_status);
-    c->launches++;
-    debug_check(st, "k_finish");
-  }
-  if (prof) CK(c, cudaEventRecord(c->ev_prof[slot][4], st));
   CK(c, cudaGetLastError());
   CK(c, cudaMemcpyAsync(&c->h_status[slot], c->d_status, sizeof(DevStatus), cudaMemcpyDeviceToHost, st));
   CK(c, cudaEventRecord(c->ev_done[slot], st));

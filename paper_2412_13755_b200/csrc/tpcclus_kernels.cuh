@@ -631,7 +631,7 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
 // lane frame with constant coefficients and rotated once.  D6's S(c) comes from the OTHER peaks
 // of the 9x9 flag window: each one adds a table entry (one nibble per owned cell it is within
 // distance 2 of, plus an "is this outer cell" bit).  The four partial sums are combined with two
-// xor-shuffles; the record is written as exact integers (RawRec) and finished by k_finish.
+// xor-shuffles; the record is staged as exact integers (RawRec) and finished by the committer warp.
 // ----------------------------------------------------------------------------------------
 constexpr int kNbrTabWords = 4 * 81;
 constexpr uint32_t kShareL = 2520u;                      // D6: lcm(1..9)
@@ -655,7 +655,7 @@ __device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
   return e;
 }
 
-struct __align__(16) RawRec {       // what k_tile writes: D7's exact integers; k_finish turns it into ClusterRec in place
+struct __align__(16) RawRec {       // what the workers stage: D7's exact integers; the committer turns it into ClusterRec
   uint32_t w0, time, w2;            // as in ClusterRec
   uint32_t W;                       // sum of weights, units of 1/(16*2520) ADC
   int32_t Mp, Mt;                   // sum w dp, sum w dt
@@ -743,29 +743,21 @@ __device__ __forceinline__ void build_cluster4(const uint16_t* __restrict__ map,
 }
 
 // ----------------------------------------------------------------------------------------
-// S5 finish (D8): RawRec -> ClusterRec in place, one thread per record.  Evaluated in double
-// from the exact integers and rounded once to float32.
+// S5 finish (D8): RawRec -> ClusterRec.  Evaluated in double from the exact integers and
+// rounded once to float32.
 // ----------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_finish(void* __restrict__ out, uint64_t out_capacity,
-                                                const DevStatus* __restrict__ status) {
-  const unsigned long long nc = status->n_clusters;
-  const uint64_t n = nc < out_capacity ? nc : out_capacity;
-  uint4* o = reinterpret_cast<uint4*>(out);
-  for (uint64_t i = uint64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += uint64_t(gridDim.x) * blockDim.x) {
-    uint4 lo = o[2 * i], hi = o[2 * i + 1];
-    const uint32_t W_ = lo.w;
-    const int32_t Mp = int32_t(hi.x), Mt = int32_t(hi.y);
-    const double Wd = double(W_);
-    const long long Np = (long long)hi.z * (long long)W_ - (long long)Mp * (long long)Mp;
-    const long long Nt = (long long)hi.w * (long long)W_ - (long long)Mt * (long long)Mt;
-    lo.w = __float_as_uint(float(Wd / 40320.0));
-    hi.x = __float_as_uint(float(double(Mp) / Wd));
-    hi.y = __float_as_uint(float(double(Mt) / Wd));
-    hi.z = __float_as_uint(float(sqrt(double(Np)) / Wd));
-    hi.w = __float_as_uint(float(sqrt(double(Nt)) / Wd));
-    o[2 * i] = lo;
-    o[2 * i + 1] = hi;
-  }
+// D8 on one record: RawRec halves -> ClusterRec halves
+__device__ __forceinline__ void finish_rec(uint4& lo, uint4& hi) {
+  const uint32_t W_ = lo.w;
+  const int32_t Mp = int32_t(hi.x), Mt = int32_t(hi.y);
+  const double Wd = double(W_);
+  const long long Np = (long long)hi.z * (long long)W_ - (long long)Mp * (long long)Mp;
+  const long long Nt = (long long)hi.w * (long long)W_ - (long long)Mt * (long long)Mt;
+  lo.w = __float_as_uint(float(Wd / 40320.0));
+  hi.x = __float_as_uint(float(double(Mp) / Wd));
+  hi.y = __float_as_uint(float(double(Mt) / Wd));
+  hi.z = __float_as_uint(float(sqrt(double(Np)) / Wd));
+  hi.w = __float_as_uint(float(sqrt(double(Nt)) / Wd));
 }
 
 // D4 on the smem map for the digit (pad, tl, q): strictly greater than the 4 neighbours earlier
@@ -836,8 +828,15 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       const uint64_t g0 = uint64_t(excl) + off;                          // first record of this item
       const uint4* src = stage + b * (2u * kListCap);
       uint4* dst = reinterpret_cast<uint4*>(P.out) + 2 * g0;
-      for (uint32_t k = lane; k < 2u * cnt; k += 32u)
-        if (g0 + (k >> 1) < P.out_capacity) dst[k] = src[k];
+      // S5 finish (D8) on this otherwise idle warp, one record per lane: fp64 from the exact integers
+      for (uint32_t r = lane; r < cnt; r += 32u) {
+        if (g0 + r < P.out_capacity) {
+          uint4 lo = src[2u * r], hi = src[2u * r + 1u];
+          finish_rec(lo, hi);
+          dst[2u * r] = lo;
+          dst[2u * r + 1u] = hi;
+        }
+      }
       bar_arrive_named(kBarEmpty + int(b), kThreads);
     }
     return;
