@@ -798,7 +798,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
-  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // [0] tile, [1] digits (next tile)
+  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // next tile: index, sector, row, tile of the row
   uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 32 * 4;        // [1..15] warp totals, [20] next peak group
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
   uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
@@ -846,15 +846,20 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   const uint32_t sub = lane & 3u;                                      // build phase: lane frame R_sub
   const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
   // address and (clamped) length of a tile's digit list (tile = bin: kTileT == kBinT)
-  auto tile_list = [&](uint32_t t, const uint32_t*& src) -> uint32_t {
-    const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
-    const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
+  auto tile_list = [&](uint32_t t, uint32_t sector, uint32_t row, uint32_t tt, const uint32_t*& src) -> uint32_t {
     const uint32_t cap = P.rows[row].cap;
     src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tt) * cap;
     return min(P.counts[t], cap);
   };
   // take the next tile in ticket order (one thread)
-  auto fetch = [&]() { s_next[0] = atomicAdd(&P.status->ticket, 1u); };
+  auto fetch = [&]() {
+    const uint32_t t = atomicAdd(&P.status->ticket, 1u);
+    const uint32_t sr = t / P.tiles_per_row, sector = sr / P.n_rows;
+    s_next[0] = t;
+    s_next[1] = sector;
+    s_next[2] = sr - sector * P.n_rows;         // row
+    s_next[3] = t - sr * P.tiles_per_row;       // tile of the row
+  };
   if (tid == 0) fetch();
   bar_sync_named(kBarWork, kWorkThreads);
 
@@ -862,8 +867,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   for (;;) {
     const uint32_t t = s_next[0];
     if (t >= P.n_tiles) break;
-    const uint32_t sr = t / P.tiles_per_row, tt = t - sr * P.tiles_per_row;
-    const uint32_t sector = sr / P.n_rows, row = sr - sector * P.n_rows;
+    const uint32_t sector = s_next[1], row = s_next[2], tt = s_next[3];
     const RowInfo ri = P.rows[row];
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
@@ -871,7 +875,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
     uint32_t* bm = reinterpret_cast<uint32_t*>(mapraw + uint32_t(kBoxH) * W * 2u);   // W % 8 == 0: 16-byte aligned
     const uint32_t* src;
-    const uint32_t n = tile_list(t, src);                                // k_bin: a multiple of 8; 0 entries are padding
+    const uint32_t n = tile_list(t, sector, row, tt, src);                                // k_bin: a multiple of 8; 0 entries are padding
     const uint4* src4 = reinterpret_cast<const uint4*>(src);
     const uint32_t n4 = n >> 2;
 
@@ -922,7 +926,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       const uint32_t tn = s_next[0];
       if (tn < P.n_tiles) {
         const uint32_t* nsrc;
-        const uint32_t nn = tile_list(tn, nsrc);
+        const uint32_t nn = tile_list(tn, s_next[1], s_next[2], s_next[3], nsrc);
         for (uint32_t i = tid * 32u; i < nn; i += kWorkThreads * 32u)
           asm volatile("prefetch.global.L2 [%0];" ::"l"(nsrc + i));
       }
@@ -943,12 +947,17 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     }
     if (lane == 31) s_misc[1 + warp] = incl;
     bar_sync_named(kBarWork, kWorkThreads);
-    uint32_t wbase = 0, total = 0;
+    uint32_t wbase, total;
+    {                                           // scan of the 15 warp totals, one per lane
+      const uint32_t v = lane < uint32_t(kWorkThreads / 32) ? s_misc[1 + lane] : 0u;
+      uint32_t ps = v;
 #pragma unroll
-    for (int w = 0; w < kWorkThreads / 32; ++w) {
-      const uint32_t v = s_misc[1 + w];
-      if (uint32_t(w) < warp) wbase += v;
-      total += v;
+      for (int o = 1; o < 16; o <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, ps, o);
+        if (lane >= uint32_t(o)) ps += u;
+      }
+      wbase = __shfl_sync(0xffffffffu, ps - v, warp);
+      total = __shfl_sync(0xffffffffu, ps, kWorkThreads / 32 - 1);
     }
     if (tid <= kTileT) rowoff[tid] = (tid < kTileT) ? (wbase + incl - cnt) : total;
     // publish the tile's count early so that later tiles' look-backs never wait for this tile's build
