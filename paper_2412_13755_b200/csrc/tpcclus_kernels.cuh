@@ -309,7 +309,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
                                                         uint32_t* __restrict__ counts, DevStatus* __restrict__ status) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   const uint32_t nb4 = (P.nb + 3u) & ~3u;
-  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  uint8_t* sp = smem_raw;                                     // __align__(128); no static shared memory before it
   uint2* stage0 = reinterpret_cast<uint2*>(sp);               sp += 2u * uint32_t(kBinChunk) * 8u;   // two TMA destinations
   uint32_t* buf = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 32u;     // 8 entries per bin
   uint32_t* cnt = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // fill count per bin
@@ -795,13 +795,12 @@ __device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
 __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ TileParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
-  uint8_t* sp = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
+  uint8_t* sp = smem_raw;                                     // __align__(128); no static shared memory before it
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
   uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // next tile: index, sector, row, tile of the row
   uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 32 * 4;        // [1..15] warp totals, [20] next peak group
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
-  uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;
   uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
   uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;
   uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 12 * 4;        // D6: L / S for S = 1..9
@@ -968,40 +967,15 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     do {
       const uint32_t b = q & 1u;
       if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
-      // rows whose peaks fit in this item: rowoff[r] + cnt - done <= kListCap (a row holds < kListCap peaks)
-      if (tid < ncore) {
-        const uint32_t ro = rowoff[tid], rn = ro + cnt;
-        if (ro >= done && rn - done <= kListCap && cnt) {
-          uint32_t k = ro - done;
-          const uint32_t* r = bm + (kReach + tid) * bmw;
-          for (uint32_t w = 0; w < bmw; ++w) {
-            uint32_t bits = r[w];
-            while (bits) {
-              const uint32_t bb = __ffs(bits) - 1;
-              bits &= bits - 1;
-              plist[k++] = ((kReach + tid) << 16) | (w * 32 + bb - 4);   // (map row, pad)
-            }
-          }
-        }
-      }
-      if (tid == 0) s_misc[20] = 0u;
-      bar_sync_named(kBarWork, kWorkThreads);
-      // peaks of this item: all that are left, or the longest prefix of whole rows that fits
-      uint32_t npass = total - done;
-      if (npass > uint32_t(kListCap)) {
-        uint32_t lo = 0, hi = ncore + 1u;            // rowoff[0..ncore] is non-decreasing, rowoff[ncore] = total
-        while (hi - lo > 1) {                        // largest row boundary <= done + kListCap
-          const uint32_t mid = (lo + hi) >> 1;
-          if (rowoff[mid] <= done + uint32_t(kListCap)) lo = mid; else hi = mid;
-        }
-        npass = rowoff[lo] - done;
-      }
+      const uint32_t npass = min(total - done, uint32_t(kListCap));
       if (tid == 0) {
+        s_misc[20] = 0u;
         s_meta[4 * b] = t;
         s_meta[4 * b + 1] = total;
         s_meta[4 * b + 2] = done;
         s_meta[4 * b + 3] = npass;
       }
+      bar_sync_named(kBarWork, kWorkThreads);                           // rowoff and the group counter are ready
       // groups of 8 peaks, four lanes per peak, taken dynamically by the worker warps
       uint4* stg = stage + b * (2u * kListCap);
       for (;;) {
@@ -1010,16 +984,38 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g * 8u >= npass) break;
         const uint32_t i = g * 8u + (lane >> 2);
-        const uint32_t e = plist[min(i, npass - 1u)];
+        // locate peak number done + i of the tile (S6 order): its row by bisection of the row offsets
+        // (the largest r with rowoff[r] <= k), then the (k - rowoff[r])-th set bit of the row's flags
+        uint32_t k = done + min(i, npass - 1u);
+        uint32_t lo = 0, hi = uint32_t(kTileT);                         // rowoff[0] = 0 <= k < total = rowoff[kTileT]
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+          const uint32_t mid = (lo + hi) >> 1;
+          if (rowoff[mid] <= k) lo = mid; else hi = mid;
+        }
+        static_assert(kTileT == 256, "eight bisection steps");
+        k -= rowoff[lo];
+        const uint32_t j = uint32_t(kReach) + lo;
+        const uint32_t* fr = bm + j * bmw;
+        uint32_t word = 0, wbit = 0;
+        bool found = false;
+        for (uint32_t w = 0; w < bmw; ++w) {
+          const uint32_t x = fr[w], c = __popc(x);
+          if (!found) {
+            if (k < c) { word = x; wbit = w * 32u; found = true; } else k -= c;
+          }
+        }
+        for (; k; --k) word &= word - 1u;                               // drop the k lowest flags
+        const uint32_t pad = wbit + uint32_t(__ffs(word)) - 1u - 4u;
         uint4 lo4, hi4;
-        build_cluster4(map, bm, nbr_tab, wtab, W, bmw, e >> 16, e & 0xFFFFu, sub, rot_cs, rot_sn, sector, row,
-                       ri.npads, t0 + int32_t(e >> 16) - kReach, P.tf_time_bins, lo4, hi4);
+        build_cluster4(map, bm, nbr_tab, wtab, W, bmw, j, pad, sub, rot_cs, rot_sn, sector, row,
+                       ri.npads, t0 + int32_t(lo), P.tf_time_bins, lo4, hi4);
         if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
       }
       bar_arrive_named(kBarFull + int(b), kThreads);
       ++q;
       done += npass;
-      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // plist and s_misc[20] are reused
+      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // the group counter is reused
     } while (done < total);
     bar_sync_named(kBarWork, kWorkThreads);   // map, bitmap and s_next are stable until here
   }
