@@ -198,7 +198,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + 16 + 32 * 4 + 2 * 4 * 4 +
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * kWinWords * 4 + 2 * kListCap * 32 + 16 + 32 * 4 + 2 * 4 * 4 + 2 * 8 * 4 +
                   (kTileT + 4) * 4 + kNbrTabWords * 4 + 12 * 4 + 128;
 
   int rc;

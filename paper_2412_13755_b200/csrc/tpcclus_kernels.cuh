@@ -26,7 +26,7 @@
 namespace tpcclus {
 
 constexpr int      kThreads      = 512;   // CTA size of k_tile (two CTAs per SM)
-constexpr int      kWorkThreads  = 480;   // warps 0..14 run S1..S5 on the tiles; warp 15 commits (look-back + copy-out)
+constexpr int      kWorkThreads  = 480;   // warps 0..14: front (0..10) and back (11..14) warps; warp 15 commits
 constexpr int      kTileT        = 256;   // core time bins per tile (= one digit bin of k_bin)
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
@@ -35,7 +35,7 @@ constexpr int      kBinShift     = 8;
 constexpr int      kBinBoxH      = kBinT + 2 * kReach;    // time rows a bin's window spans (266)
 static_assert((1 << kBinShift) == kBinT && kBinT == kTileT, "a digit bin is one tile");
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
-constexpr int      kListCap      = 136;   // peaks per hand-over item (capacity of one staging buffer; > 128 = most peaks of a row)
+constexpr int      kListCap      = 96;    // peaks per hand-over item (capacity of one window / staging buffer)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 
@@ -663,33 +663,59 @@ struct __align__(16) RawRec {       // what the workers stage: D7's exact intege
 };
 static_assert(sizeof(RawRec) == 32, "raw record is 32 bytes");
 
-// All 32 lanes call this; lanes 4g..4g+3 work on the same peak (j = map row, pad).  Returns the
-// two 16-byte halves of the RawRec in every lane of the group.
-__device__ __forceinline__ void build_cluster4(const uint16_t* __restrict__ map, const uint32_t* __restrict__ bm,
-                                               const uint32_t* __restrict__ nbr_tab, const uint32_t* __restrict__ wtab,
-                                               uint32_t W, uint32_t bmw, uint32_t j, uint32_t pad, uint32_t sub,
-                                               int32_t cs, int32_t sn, uint32_t sector, uint32_t row, uint32_t npads,
-                                               int32_t tglob, uint32_t tf_time_bins, uint4& lo, uint4& hi) {
+// A peak's WINDOW: what S3..S5 need of the tile's map and flags, 80 bytes.  The front warps cut it
+// out (four lanes per peak) so that the map can be reused for the next tile while the back warps
+// still build this tile's clusters.  Layout (5 x uint4): [lane frame 0..3: the 8 charges
+// qP|qIm, qI0|qI1, qO0|qO1, qO2|qO3 as u16 pairs] [G0, G1, G2, j<<16 | pad] with the 9x9 flag
+// window packed three rows per word: bit 9*(k%3)+i of G[k/3] <-> row j-4+k, pad p-4+i, P cleared.
+constexpr int kWinWords = 20;
+
+// All 32 lanes call this; lanes 4g..4g+3 work on the same peak (j = map row, pad).
+__device__ __forceinline__ void extract_window4(const uint16_t* __restrict__ map, const uint32_t* __restrict__ bm,
+                                                uint32_t W, uint32_t bmw, uint32_t j, uint32_t pad, uint32_t sub,
+                                                int32_t cs, int32_t sn, uint4* __restrict__ win) {
   const uint16_t* c = map + j * W + (pad + kColOff);
   const int32_t X = sn * int32_t(W) + cs, Y = cs * int32_t(W) - sn;     // steps of (a,b) in map cells
   const uint32_t qP = c[0];
   const uint32_t qIm = c[X - Y], qI0 = c[X], qI1 = c[X + Y];
   const uint32_t qO0 = c[2 * X - Y], qO1 = c[2 * X], qO2 = c[2 * X + Y], qO3 = c[2 * X + 2 * Y];
-
-  // 9x9 flag window packed three rows per word: bit 9*(k%3)+i of G[k/3] <-> row j-4+k, pad p-4+i
+  win[sub] = make_uint4(qP | (qIm << 16), qI0 | (qI1 << 16), qO0 | (qO1 << 16), qO2 | (qO3 << 16));
+  // flag rows: lane s reads rows s and s+4, lane 0 also row 8; OR-combined over the four lanes
   uint32_t G0 = 0, G1 = 0, G2 = 0;
   {
     const uint32_t sh = pad & 31u;
     const uint32_t* rowp = bm + (j - 4u) * bmw + (pad >> 5);
+    auto row_bits = [&](uint32_t k) -> uint32_t {
+      return __funnelshift_r(rowp[k * bmw], rowp[k * bmw + 1], sh) & 0x1FFu;
+    };
+    const uint32_t fa = row_bits(sub), fb = row_bits(sub + 4u), fc = sub == 0u ? row_bits(8u) : 0u;
+    // row k -> word k/3, shift 9*(k%3)
+    if (sub < 3u) G0 = fa << (9u * sub); else G1 = fa;                   // rows 0,1,2 | 3
+    if (sub < 2u) G1 |= fb << (9u * (sub + 1u)); else G2 = fb << (9u * (sub - 2u));   // rows 4,5 | 6,7
+    G2 |= fc << 18;                                                      // row 8
 #pragma unroll
-    for (int k = 0; k < 9; ++k) {
-      const uint32_t f = __funnelshift_r(rowp[k * bmw], rowp[k * bmw + 1], sh) & 0x1FFu;
-      if (k < 3) G0 |= f << (9 * k);
-      else if (k < 6) G1 |= f << (9 * (k - 3));
-      else G2 |= f << (9 * (k - 6));
+    for (int o = 1; o <= 2; o <<= 1) {
+      G0 |= __shfl_xor_sync(0xffffffffu, G0, o);
+      G1 |= __shfl_xor_sync(0xffffffffu, G1, o);
+      G2 |= __shfl_xor_sync(0xffffffffu, G2, o);
     }
     G1 &= ~(1u << 13);                                                  // P itself (row 4, column 4)
   }
+  if (sub == 3u) win[4] = make_uint4(G0, G1, G2, (j << 16) | pad);
+}
+
+// All 32 lanes call this; lanes 4g..4g+3 assemble the cluster of one window.  Returns the two
+// 16-byte halves of the RawRec in every lane of the group.
+__device__ __forceinline__ void assemble4(const uint4* __restrict__ win, const uint32_t* __restrict__ nbr_tab,
+                                          const uint32_t* __restrict__ wtab, uint32_t sub, int32_t cs, int32_t sn,
+                                          uint32_t sector_row /* sector | row << 8 */, uint32_t npads, int32_t t_row0,
+                                          uint32_t tf_time_bins, uint4& lo, uint4& hi) {
+  const uint4 ch = win[sub], fl = win[4];
+  const uint32_t qP = ch.x & 0xFFFFu, qIm = ch.x >> 16, qI0 = ch.y & 0xFFFFu, qI1 = ch.y >> 16;
+  const uint32_t qO0 = ch.z & 0xFFFFu, qO1 = ch.z >> 16, qO2 = ch.w & 0xFFFFu, qO3 = ch.w >> 16;
+  uint32_t G0 = fl.x, G1 = fl.y, G2 = fl.z;
+  const uint32_t pad = fl.w & 0xFFFFu;
+  const int32_t tglob = t_row0 + int32_t(fl.w >> 16);                  // t_row0 = global time of map row 0
   uint32_t acc = 0;                                                     // nibble c: other peaks within distance 2 of cell c
   {
     const uint32_t* t = nbr_tab + sub * 81u;
@@ -737,7 +763,7 @@ __device__ __forceinline__ void build_cluster4(const uint16_t* __restrict__ map,
   if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
   if (qP == kQClamp || (meta & 0xFF00u)) flags |= 4u;                   // SATURATED
   if (meta >> 16) flags |= 8u;                                          // SPLIT
-  lo = make_uint4(sector | (row << 8) | (pad << 16) | (flags << 24), uint32_t(tglob),
+  lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob),
                   qP | (((meta & 0xFFu) + 1u) << 16), Wsum);
   hi = make_uint4(uint32_t(Mp), uint32_t(Mt), Mpp, Mtt);
 }
@@ -778,15 +804,22 @@ __device__ __forceinline__ bool is_peak(const uint32_t* __restrict__ map32, uint
   return q > early && q >= late;
 }
 
-// Worker / committer pipeline.  Warps 0..6 (the workers) take tiles by ticket and run S1..S5
-// on them; the RawRecs of a tile are written to one of two shared-memory staging buffers and
-// handed to warp 7 (the committer), which runs the decoupled look-back of the tile (S6) and
-// copies the records to their final position while the workers are already on the next tile.
-// Hand-over is by named barriers (bar.arrive / bar.sync, 256 participants each):
-//   kBarFull + b   workers arrive, committer syncs : staging[b] and meta[b] are written
-//   kBarEmpty + b  committer arrives, workers sync : staging[b] has been copied out
-// A tile with more peaks than the staging buffer holds is handed over in several items.
-constexpr int kBarWork = 1, kBarFull = 2, kBarEmpty = 4;
+// Front / back / committer pipeline inside one CTA of 16 warps:
+//   front  (warps 0..10)  take tiles by ticket; zero the map, scatter the list (S1), D4 peak flags
+//                         (S2), count + scan (S6 in-tile part), then cut each peak's WINDOW out of
+//                         the map and flags into one of two window buffers — and go on to the next
+//                         tile at once: nothing after this point needs the map
+//   back   (warps 11..14) S3..S5 from the windows, four lanes per peak; RawRecs into one of two
+//                         staging buffers
+//   committer (warp 15)   decoupled look-back of the tile (S6), D8 finish, copy-out
+// Hand-over is by named barriers (bar.arrive by the producers, bar.sync by the consumers):
+//   kBarWinFull + b / kBarWinEmpty + b   front <-> back      (window buffer b and wmeta[b])
+//   kBarFull + b    / kBarEmpty + b      back  <-> committer (staging buffer b and s_meta[b])
+// A tile with more peaks than a buffer holds is handed over in several items; a tile without
+// peaks still sends one empty item (its look-back has to publish a prefix).
+constexpr int kFrontThreads = 352, kBackThreads = 128;
+static_assert(kFrontThreads + kBackThreads == kWorkThreads && kFrontThreads >= kTileT + 1, "role split");
+constexpr int kBarWork = 1, kBarFull = 2, kBarEmpty = 4, kBarWinFull = 6, kBarWinEmpty = 8;
 constexpr uint32_t kStopTile = 0xFFFFFFFFu;
 __device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
@@ -797,10 +830,12 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   // carve-up
   uint8_t* sp = smem_raw;                                     // __align__(128); no static shared memory before it
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bitmap
+  uint4* wins = reinterpret_cast<uint4*>(sp);               sp += 2 * kListCap * kWinWords * 4;   // two window buffers
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
   uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // next tile: index, sector, row, tile of the row
-  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 32 * 4;        // [1..15] warp totals, [20] next peak group
+  uint32_t* s_misc = reinterpret_cast<uint32_t*>(sp);       sp += 32 * 4;        // [1..11] warp totals, [20] next peak group
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
+  uint32_t* wmeta = reinterpret_cast<uint32_t*>(sp);        sp += 2 * 8 * 4;     // per window buffer: + sector|row<<8, npads, time of map row 0
   uint32_t* rowoff = reinterpret_cast<uint32_t*>(sp);       sp += (kTileT + 4) * 4;
   uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;
   uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 12 * 4;        // D6: L / S for S = 1..9
@@ -810,13 +845,15 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   for (uint32_t i = tid; i < uint32_t(kNbrTabWords); i += kThreads) nbr_tab[i] = nbr_tab_entry(i);
   if (tid < 9u) wtab[tid] = kShareL / (tid + 1u);
   __syncthreads();
+  const uint32_t sub = lane & 3u;                                      // four lanes per peak: lane frame R_sub
+  const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
 
   if (warp == uint32_t(kWorkThreads / 32)) {
-    // ================= committer warp: S6 look-back + copy-out =================
+    // ================= committer warp: S6 look-back, S5 finish, copy-out =================
     uint32_t excl = 0;
     for (uint32_t q = 0;; ++q) {
       const uint32_t b = q & 1u;
-      bar_sync_named(kBarFull + int(b), kThreads);
+      bar_sync_named(kBarFull + int(b), kBackThreads + 32);
       const uint32_t t = s_meta[4 * b];
       if (t == kStopTile) break;
       const uint32_t total = s_meta[4 * b + 1], off = s_meta[4 * b + 2], cnt = s_meta[4 * b + 3];
@@ -827,7 +864,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       const uint64_t g0 = uint64_t(excl) + off;                          // first record of this item
       const uint4* src = stage + b * (2u * kListCap);
       uint4* dst = reinterpret_cast<uint4*>(P.out) + 2 * g0;
-      // S5 finish (D8) on this otherwise idle warp, one record per lane: fp64 from the exact integers
+      // S5 finish (D8), one record per lane: fp64 from the exact integers
       for (uint32_t r = lane; r < cnt; r += 32u) {
         if (g0 + r < P.out_capacity) {
           uint4 lo = src[2u * r], hi = src[2u * r + 1u];
@@ -836,14 +873,49 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
           dst[2u * r + 1u] = hi;
         }
       }
-      bar_arrive_named(kBarEmpty + int(b), kThreads);
+      bar_arrive_named(kBarEmpty + int(b), kBackThreads + 32);
     }
     return;
   }
 
-  // ================= worker warps =================
-  const uint32_t sub = lane & 3u;                                      // build phase: lane frame R_sub
-  const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
+  if (warp >= uint32_t(kFrontThreads / 32)) {
+    // ================= back warps: S3..S5 from the windows =================
+    const uint32_t bw = warp - uint32_t(kFrontThreads / 32);            // 0..3
+    const uint32_t btid = tid - uint32_t(kFrontThreads);
+    for (uint32_t q = 0;; ++q) {
+      const uint32_t b = q & 1u;
+      bar_sync_named(kBarWinFull + int(b), kWorkThreads);               // window buffer b and wmeta[b] are written
+      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kBackThreads + 32);   // staging[b] has been copied out
+      const uint32_t* m = wmeta + 8u * b;
+      const uint32_t t = m[0];
+      if (btid == 0) {
+        s_meta[4 * b] = t;
+        s_meta[4 * b + 1] = m[1];
+        s_meta[4 * b + 2] = m[2];
+        s_meta[4 * b + 3] = m[3];
+      }
+      if (t == kStopTile) {
+        bar_arrive_named(kBarFull + int(b), kBackThreads + 32);
+        break;
+      }
+      const uint32_t npass = m[3], sector_row = m[4], npads = m[5];
+      const int32_t t_row0 = int32_t(m[6]);
+      const uint4* wb = wins + b * uint32_t(kListCap * kWinWords / 4);
+      uint4* stg = stage + b * (2u * kListCap);
+      for (uint32_t g = bw; g * 8u < npass; g += uint32_t(kBackThreads / 32)) {
+        const uint32_t i = g * 8u + (lane >> 2);
+        uint4 lo4, hi4;
+        assemble4(wb + min(i, npass - 1u) * uint32_t(kWinWords / 4), nbr_tab, wtab, sub, rot_cs, rot_sn, sector_row,
+                  npads, t_row0, P.tf_time_bins, lo4, hi4);
+        if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
+      }
+      bar_arrive_named(kBarWinEmpty + int(b), kWorkThreads);            // the windows are consumed
+      bar_arrive_named(kBarFull + int(b), kBackThreads + 32);           // the records are staged
+    }
+    return;
+  }
+
+  // ================= front warps: S1, S2, in-tile S6, window cut-out =================
   // address and (clamped) length of a tile's digit list (tile = bin: kTileT == kBinT)
   auto tile_list = [&](uint32_t t, uint32_t sector, uint32_t row, uint32_t tt, const uint32_t*& src) -> uint32_t {
     const uint32_t cap = P.rows[row].cap;
@@ -860,7 +932,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     s_next[3] = t - sr * P.tiles_per_row;       // tile of the row
   };
   if (tid == 0) fetch();
-  bar_sync_named(kBarWork, kWorkThreads);
+  bar_sync_named(kBarWork, kFrontThreads);
 
   uint32_t q = 0;                                                      // hand-over items issued so far
   for (;;) {
@@ -882,9 +954,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     {
       const uint32_t nz = (uint32_t(kBoxH) * W * 2u + uint32_t(kBoxH) * bmw * 4u + 15u) >> 4;
       uint4* z = reinterpret_cast<uint4*>(mapraw);
-      for (uint32_t i = tid; i < nz; i += kWorkThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+      for (uint32_t i = tid; i < nz; i += kFrontThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
-    bar_sync_named(kBarWork, kWorkThreads);
+    bar_sync_named(kBarWork, kFrontThreads);
     if (tid == 0) fetch();                    // next tile's ticket (s_next is read again after later barriers)
 
     // ---- S1: scatter the list into the map (16-byte streaming loads, two in flight per thread) ----
@@ -893,8 +965,8 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         if (d) map[dig_tl(d) * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
       };
       uint32_t i = tid;
-      for (; i + kWorkThreads < n4; i += 2 * kWorkThreads) {
-        const uint4 a = __ldg(src4 + i), c = __ldg(src4 + i + kWorkThreads);
+      for (; i + kFrontThreads < n4; i += 2 * kFrontThreads) {
+        const uint4 a = __ldg(src4 + i), c = __ldg(src4 + i + kFrontThreads);
         put(a.x); put(a.y); put(a.z); put(a.w);
         put(c.x); put(c.y); put(c.z); put(c.w);
       }
@@ -904,7 +976,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       }
       if (tid < (n & 3u)) put(__ldg(src + 4u * n4 + tid));               // k_bin_direct lists: any length
     }
-    bar_sync_named(kBarWork, kWorkThreads);
+    bar_sync_named(kBarWork, kFrontThreads);
 
     // ---- S2: D4 peak flags for map rows 1..kBoxH-2, digit-driven (the list is in L1/L2 now) ----
     {
@@ -914,7 +986,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
           atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
       };
-      for (uint32_t i = tid; i < n4; i += kWorkThreads) {
+      for (uint32_t i = tid; i < n4; i += kFrontThreads) {
         const uint4 a = __ldg(src4 + i);
         test(a.x); test(a.y); test(a.z); test(a.w);
       }
@@ -926,11 +998,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       if (tn < P.n_tiles) {
         const uint32_t* nsrc;
         const uint32_t nn = tile_list(tn, s_next[1], s_next[2], s_next[3], nsrc);
-        for (uint32_t i = tid * 32u; i < nn; i += kWorkThreads * 32u)
+        for (uint32_t i = tid * 32u; i < nn; i += kFrontThreads * 32u)
           asm volatile("prefetch.global.L2 [%0];" ::"l"(nsrc + i));
       }
     }
-    bar_sync_named(kBarWork, kWorkThreads);   // flags complete
+    bar_sync_named(kBarWork, kFrontThreads);   // flags complete
 
     // ---- S6 (in-tile part): ordered count of the core rows, block scan ----
     uint32_t cnt = 0;
@@ -945,10 +1017,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       if (lane >= uint32_t(o)) incl += v;
     }
     if (lane == 31) s_misc[1 + warp] = incl;
-    bar_sync_named(kBarWork, kWorkThreads);
+    bar_sync_named(kBarWork, kFrontThreads);
     uint32_t wbase, total;
     {                                           // scan of the 15 warp totals, one per lane
-      const uint32_t v = lane < uint32_t(kWorkThreads / 32) ? s_misc[1 + lane] : 0u;
+      const uint32_t v = lane < uint32_t(kFrontThreads / 32) ? s_misc[1 + lane] : 0u;
       uint32_t ps = v;
 #pragma unroll
       for (int o = 1; o < 16; o <<= 1) {
@@ -956,37 +1028,41 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         if (lane >= uint32_t(o)) ps += u;
       }
       wbase = __shfl_sync(0xffffffffu, ps - v, warp);
-      total = __shfl_sync(0xffffffffu, ps, kWorkThreads / 32 - 1);
+      total = __shfl_sync(0xffffffffu, ps, kFrontThreads / 32 - 1);
     }
     if (tid <= kTileT) rowoff[tid] = (tid < kTileT) ? (wbase + incl - cnt) : total;
     // publish the tile's count early so that later tiles' look-backs never wait for this tile's build
     if (tid == 0 && t != 0u) st_release_u64(P.tile_state + t, pack_state(P.epoch, kStAgg, total));
 
-    // ---- S3..S5: clusters, at most kListCap peaks per hand-over item ----
+    // ---- window cut-out, at most kListCap peaks per hand-over item ----
     uint32_t done = 0;
     do {
       const uint32_t b = q & 1u;
-      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
+      if (q >= 2u) bar_sync_named(kBarWinEmpty + int(b), kFrontThreads + kBackThreads);   // the back warps are done with buffer b
       const uint32_t npass = min(total - done, uint32_t(kListCap));
       if (tid == 0) {
         s_misc[20] = 0u;
-        s_meta[4 * b] = t;
-        s_meta[4 * b + 1] = total;
-        s_meta[4 * b + 2] = done;
-        s_meta[4 * b + 3] = npass;
+        uint32_t* m = wmeta + 8u * b;
+        m[0] = t;
+        m[1] = total;
+        m[2] = done;
+        m[3] = npass;
+        m[4] = sector | (row << 8);
+        m[5] = ri.npads;
+        m[6] = uint32_t(t0 - kReach);                                   // global time of map row 0
       }
-      bar_sync_named(kBarWork, kWorkThreads);                           // rowoff and the group counter are ready
-      // groups of 8 peaks, four lanes per peak, taken dynamically by the worker warps
-      uint4* stg = stage + b * (2u * kListCap);
+      bar_sync_named(kBarWork, kFrontThreads);                          // rowoff and the group counter are ready
+      // groups of 8 peaks, four lanes per peak, taken dynamically by the front warps
+      uint4* wb = wins + b * uint32_t(kListCap * kWinWords / 4);
       for (;;) {
         uint32_t g = 0;
         if (lane == 0) g = atomicAdd(&s_misc[20], 1u);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g * 8u >= npass) break;
-        const uint32_t i = g * 8u + (lane >> 2);
+        const uint32_t i = min(g * 8u + (lane >> 2), npass - 1u);      // (a ragged group redoes the item's last peak)
         // locate peak number done + i of the tile (S6 order): its row by bisection of the row offsets
         // (the largest r with rowoff[r] <= k), then the (k - rowoff[r])-th set bit of the row's flags
-        uint32_t k = done + min(i, npass - 1u);
+        uint32_t k = done + i;
         uint32_t lo = 0, hi = uint32_t(kTileT);                         // rowoff[0] = 0 <= k < total = rowoff[kTileT]
 #pragma unroll
         for (int it = 0; it < 8; ++it) {
@@ -1007,25 +1083,21 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         }
         for (; k; --k) word &= word - 1u;                               // drop the k lowest flags
         const uint32_t pad = wbit + uint32_t(__ffs(word)) - 1u - 4u;
-        uint4 lo4, hi4;
-        build_cluster4(map, bm, nbr_tab, wtab, W, bmw, j, pad, sub, rot_cs, rot_sn, sector, row,
-                       ri.npads, t0 + int32_t(lo), P.tf_time_bins, lo4, hi4);
-        if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
+        extract_window4(map, bm, W, bmw, j, pad, sub, rot_cs, rot_sn, wb + i * uint32_t(kWinWords / 4));
       }
-      bar_arrive_named(kBarFull + int(b), kThreads);
+      bar_arrive_named(kBarWinFull + int(b), kFrontThreads + kBackThreads);
       ++q;
       done += npass;
-      if (done < total) bar_sync_named(kBarWork, kWorkThreads);        // the group counter is reused
+      if (done < total) bar_sync_named(kBarWork, kFrontThreads);       // the group counter is reused
     } while (done < total);
-    bar_sync_named(kBarWork, kWorkThreads);   // map, bitmap and s_next are stable until here
+    bar_sync_named(kBarWork, kFrontThreads);   // map, bitmap and s_next are stable until here
   }
-  // stop item, then wait until the committer has drained the last real item
+  // stop item: the back warps pass it on to the committer
   {
     const uint32_t b = q & 1u;
-    if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);
-    if (tid == 0) s_meta[4 * b] = kStopTile;
-    bar_arrive_named(kBarFull + int(b), kThreads);
-    if (q >= 1u) bar_sync_named(kBarEmpty + int((q - 1u) & 1u), kThreads);
+    if (q >= 2u) bar_sync_named(kBarWinEmpty + int(b), kFrontThreads + kBackThreads);
+    if (tid == 0) wmeta[8u * b] = kStopTile;
+    bar_arrive_named(kBarWinFull + int(b), kFrontThreads + kBackThreads);
   }
 }
 
