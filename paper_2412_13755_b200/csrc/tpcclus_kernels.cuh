@@ -25,8 +25,8 @@
 
 namespace tpcclus {
 
-constexpr int      kThreads      = 512;   // CTA size of k_tile (two CTAs per SM)
-constexpr int      kWorkThreads  = 480;   // warps 0..14: front (0..10) and back (11..14) warps; warp 15 commits
+constexpr int      kThreads      = 640;   // CTA size of k_tile (two CTAs per SM)
+constexpr int      kWorkThreads  = 608;   // warps 0..18: front (0..14) and back (15..18) warps; warp 19 commits
 constexpr int      kTileT        = 256;   // core time bins per tile (= one digit bin of k_bin)
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (138)
@@ -804,20 +804,20 @@ __device__ __forceinline__ bool is_peak(const uint32_t* __restrict__ map32, uint
   return q > early && q >= late;
 }
 
-// Front / back / committer pipeline inside one CTA of 16 warps:
-//   front  (warps 0..10)  take tiles by ticket; zero the map, scatter the list (S1), D4 peak flags
+// Front / back / committer pipeline inside one CTA of 20 warps:
+//   front  (warps 0..14)  take tiles by ticket; zero the map, scatter the list (S1), D4 peak flags
 //                         (S2), count + scan (S6 in-tile part), then cut each peak's WINDOW out of
 //                         the map and flags into one of two window buffers — and go on to the next
 //                         tile at once: nothing after this point needs the map
-//   back   (warps 11..14) S3..S5 from the windows, four lanes per peak; RawRecs into one of two
+//   back   (warps 15..18) S3..S5 from the windows, four lanes per peak; RawRecs into one of two
 //                         staging buffers
-//   committer (warp 15)   decoupled look-back of the tile (S6), D8 finish, copy-out
+//   committer (warp 19)   decoupled look-back of the tile (S6), D8 finish, copy-out
 // Hand-over is by named barriers (bar.arrive by the producers, bar.sync by the consumers):
 //   kBarWinFull + b / kBarWinEmpty + b   front <-> back      (window buffer b and wmeta[b])
 //   kBarFull + b    / kBarEmpty + b      back  <-> committer (staging buffer b and s_meta[b])
 // A tile with more peaks than a buffer holds is handed over in several items; a tile without
 // peaks still sends one empty item (its look-back has to publish a prefix).
-constexpr int kFrontThreads = 352, kBackThreads = 128;
+constexpr int kFrontThreads = 480, kBackThreads = 128;
 static_assert(kFrontThreads + kBackThreads == kWorkThreads && kFrontThreads >= kTileT + 1, "role split");
 constexpr int kBarWork = 1, kBarFull = 2, kBarEmpty = 4, kBarWinFull = 6, kBarWinEmpty = 8;
 constexpr uint32_t kStopTile = 0xFFFFFFFFu;
@@ -1023,7 +1023,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       const uint32_t v = lane < uint32_t(kFrontThreads / 32) ? s_misc[1 + lane] : 0u;
       uint32_t ps = v;
 #pragma unroll
-      for (int o = 1; o < 16; o <<= 1) {
+      for (int o = 1; o < 32; o <<= 1) {
         const uint32_t u = __shfl_up_sync(0xffffffffu, ps, o);
         if (lane >= uint32_t(o)) ps += u;
       }
