@@ -981,16 +981,26 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     // ---- S2: D4 peak flags for map rows 1..kBoxH-2, digit-driven (the list is in L1/L2 now) ----
     {
       const uint32_t* map32 = reinterpret_cast<const uint32_t*>(map);
-      auto test = [&](uint32_t d) {
-        const uint32_t q16 = dig_q(d), tl = dig_tl(d), pad = dig_pad(d);
-        if (q16 >= P.theta && tl - 1u < uint32_t(kBoxH - 2) && is_peak(map32, wpr, pad, tl, q16))
-          atomicOr(&bm[tl * bmw + ((pad + 4u) >> 5)], 1u << ((pad + 4u) & 31u));
+      // branch-free up to the flag store, so that the loads of several entries overlap: an entry that
+      // cannot be a peak (below theta, halo row 0 / last, padding) is tested at a harmless cell instead
+      auto test2 = [&](uint32_t d0, uint32_t d1) {
+        uint32_t q0 = dig_q(d0), tl0 = dig_tl(d0), pad0 = dig_pad(d0);
+        uint32_t q1 = dig_q(d1), tl1 = dig_tl(d1), pad1 = dig_pad(d1);
+        const bool ok0 = q0 >= P.theta && tl0 - 1u < uint32_t(kBoxH - 2);
+        const bool ok1 = q1 >= P.theta && tl1 - 1u < uint32_t(kBoxH - 2);
+        if (!ok0) { tl0 = 1u; pad0 = 0u; }
+        if (!ok1) { tl1 = 1u; pad1 = 0u; }
+        const bool p0 = is_peak(map32, wpr, pad0, tl0, q0);
+        const bool p1 = is_peak(map32, wpr, pad1, tl1, q1);
+        if (ok0 && p0) atomicOr(&bm[tl0 * bmw + ((pad0 + 4u) >> 5)], 1u << ((pad0 + 4u) & 31u));
+        if (ok1 && p1) atomicOr(&bm[tl1 * bmw + ((pad1 + 4u) >> 5)], 1u << ((pad1 + 4u) & 31u));
       };
       for (uint32_t i = tid; i < n4; i += kFrontThreads) {
         const uint4 a = __ldg(src4 + i);
-        test(a.x); test(a.y); test(a.z); test(a.w);
+        test2(a.x, a.y);
+        test2(a.z, a.w);
       }
-      if (tid < (n & 3u)) test(__ldg(src + 4u * n4 + tid));
+      if (tid < (n & 3u)) test2(__ldg(src + 4u * n4 + tid), 0u);
     }
     // pull the next tile's list towards L2 while this tile is counted and built
     {
