@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256) k_bin_direct(const uint2* __restrict__ di
 // Why: appending digits one by one costs one scattered 4-byte store per list entry and, even
 // when a CTA aggregates a chunk's reservations, about one global atomic per 2-4 entries; ncu
 // shows both k_bin_direct and the chunk-aggregated variant pinned at ~45 % L1/L2 transaction
-// throughput with every warp waiting (profiles/r1c_*).  Here each CTA (one per SM) keeps an
+// throughput with every warp waiting (profiles/r1c_bin_ncu.md).  Here each CTA (one per SM) keeps an
 // 8-entry (32-byte = one DRAM sector) buffer per bin of the sector it is reading in shared
 // memory, and a bin costs ONE global atomic and ONE aligned 32-byte store per 8 entries:
 //   A   every digit of the chunk (TMA-staged, double-buffered): quantise (D1), validate, rank
