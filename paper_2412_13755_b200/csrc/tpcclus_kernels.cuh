@@ -298,7 +298,7 @@ constexpr uint32_t kBinNone     = 0xFFFFFFFFu;              // staging slot with
 
 __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
   const uint32_t nb4 = (nb + 3u) & ~3u;
-  return 2u * uint32_t(kBinChunk) * 8u + nb4 * 32u + nb4 * 4u + nb4 * 4u + nb4 * 2u + uint32_t(kBinSecCap) * 8u +
+  return 2u * uint32_t(kBinChunk) * 8u + nb4 * 32u + nb4 * 4u + nb4 * 4u + nb4 * 4u + nb4 * 2u + uint32_t(kBinSecCap) * 8u +
          3u * 256u * 4u + 96u + 128u;
 }
 
@@ -322,6 +322,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   uint32_t* s_par = reinterpret_cast<uint32_t*>(sp);          sp += 32;            // per staging buffer: sector, slot_lo, slot_hi
   uint32_t* dst = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // list offset of the bin's last reservation
   uint16_t* nfull = reinterpret_cast<uint16_t*>(sp);          sp += nb4 * 2u;      // whole sectors of that reservation
+  uint32_t* nxt = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // list offset of the sector reserved ahead for the bin
 
   const uint32_t tid = threadIdx.x;
   for (uint32_t i = tid; i < 256u; i += kBinThreads) {
@@ -392,21 +393,47 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   };
   const uint32_t bpr = P.bins_per_row;
   const uint32_t t_span = uint32_t(P.t_hi - P.t_lo);
-  // flush every partly filled buffer of sector s (padded with zero entries to a whole sector)
+  // phase B1 visits bins tid, tid + 1024, ... (P.nb <= 4 * kBinThreads): their list offsets and
+  // capacities never change, and each keeps ONE SECTOR RESERVED AHEAD (nxt[bin]) so that a flush is
+  // a plain store; the reservation that replaces it is an atomic whose result (res_g, valid in
+  // res_m) is only looked at one chunk later — its latency is never waited for.
+  uint32_t b_off[4], b_cap[4], res_g[4] = {0u, 0u, 0u, 0u}, res_m = 0u;
+  auto apply_reservations = [&]() {
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+      if (res_m & (1u << x))
+        nxt[tid + uint32_t(x) * kBinThreads] = (res_g[x] + 8u <= b_cap[x]) ? b_off[x] + res_g[x] : kBinFull;
+    res_m = 0u;
+  };
+  // entering sector s: one sector reserved for every bin
+  auto reserve_all = [&](uint32_t s) {
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const uint32_t bin = tid + uint32_t(x) * kBinThreads;
+      if (bin < P.nb) {
+        res_g[x] = atomicAdd(&counts[s * P.nb + bin], 8u);
+        res_m |= 1u << x;
+      }
+    }
+    apply_reservations();
+  };
+  // leaving sector s: every bin's partly filled buffer goes to its reserved sector, zero-padded
+  // (an empty buffer too: the sector is part of the list now and must not keep stale entries)
   auto flush_all = [&](uint32_t s) {
     uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
-    for (uint32_t bin = tid; bin < P.nb; bin += kBinThreads) {
-      const uint32_t n = cnt[bin];                            // < 8: fuller bins were flushed in phase B1
-      if (n) {
-        for (uint32_t x = n; x < 8u; ++x) buf[bin * 8u + x] = 0u;
+    apply_reservations();
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const uint32_t bin = tid + uint32_t(x) * kBinThreads;
+      if (bin < P.nb) {
+        const uint32_t n = cnt[bin];                          // < 8: fuller bins were flushed in phase B1
+        for (uint32_t y = n; y < 8u; ++y) buf[bin * 8u + y] = 0u;
         const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
-        const uint32_t row = bin / bpr, tb = bin - row * bpr, cap = r_cap[row];
-        const uint32_t base = atomicAdd(&counts[s * P.nb + bin], 8u);
-        if (base + 8u <= cap) {
-          uint32_t* d = seclist + r_off[row] + tb * cap + base;
-          st_v4(d, a);
-          st_v4(d + 4, c);
+        const uint32_t d = nxt[bin];
+        if (d != kBinFull) {
+          st_v4(seclist + d, a);
+          st_v4(seclist + d + 4, c);
         }
         cnt[bin] = 0u;
       }
@@ -420,8 +447,6 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     if (tid == 0) load(k0, s, 0);
   }
   __syncthreads();
-  // phase B1 visits bins tid, tid + 1024, ...: their list offsets and capacities never change
-  uint32_t b_off[4], b_cap[4];
 #pragma unroll
   for (int x = 0; x < 4; ++x) {
     const uint32_t bin = tid + uint32_t(x) * kBinThreads;
@@ -429,6 +454,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     b_cap[x] = r_cap[row];
     b_off[x] = r_off[row] + tb * b_cap[x];
   }
+  if (k0 < k1) reserve_all(s);
   for (uint32_t k = k0; k < k1; ++k) {
     const uint32_t b = (k - k0) & 1u;
     {
@@ -436,6 +462,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
       if (s_new != s) {
         flush_all(s);
         s = s_new;
+        reserve_all(s);
       }
     }
     if (tid == 0 && k + 1 < k1) load(k + 1, sector_of(k + 1, s), b ^ 1u);   // lands while this chunk is processed
@@ -502,35 +529,31 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     }
     __syncthreads();                  // every entry is ranked; buffers and counts are complete
 
-    // ---- phase B1: bins holding a whole sector: reserve the whole sectors (one global atomic per
-    //      bin, up to four in flight per thread), store the buffered sector, keep the remainder ----
+    // ---- phase B1: bins holding a whole sector: store it into the sector reserved ahead, request the
+    //      next reservation (one global atomic per flush, never waited for), keep the remainder ----
     if (tid == 0) s_ctl[b ^ 1u] = 0u; // the other buffer's counter is idle until the next chunk's phase A
-    {                                 // P.nb <= kBinMaxNb = 4 * kBinThreads
-      uint32_t n[4], g[4];
+    apply_reservations();             // (issued in the previous chunk's phase B1)
 #pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        const uint32_t bin = tid + uint32_t(x) * kBinThreads;
-        n[x] = bin < P.nb ? cnt[bin] : 0u;
-      }
-#pragma unroll
-      for (int x = 0; x < 4; ++x)
-        g[x] = n[x] >= 8u ? atomicAdd(&counts[cbase + tid + uint32_t(x) * kBinThreads], n[x] & ~7u) : 0u;
-#pragma unroll
-      for (int x = 0; x < 4; ++x) {
-        if (n[x] >= 8u) {
-          const uint32_t bin = tid + uint32_t(x) * kBinThreads;
-          const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
-          const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
-          uint32_t d = kBinFull;
-          if (g[x] + (n[x] & ~7u) <= b_cap[x]) {
-            d = b_off[x] + g[x];
-            st_v4(seclist + d, a);
-            st_v4(seclist + d + 4, c);
-          }
-          dst[bin] = d;
-          nfull[bin] = uint16_t(n[x] >> 3);
-          cnt[bin] = n[x] & 7u;       // entries ranked >= 8 * nfull move to the buffer's front in phase B2
+    for (int x = 0; x < 4; ++x) {
+      const uint32_t bin = tid + uint32_t(x) * kBinThreads;
+      const uint32_t n = bin < P.nb ? cnt[bin] : 0u;
+      if (n >= 8u) {
+        const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
+        const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
+        const uint32_t d = nxt[bin];
+        if (d != kBinFull) {
+          st_v4(seclist + d, a);
+          st_v4(seclist + d + 4, c);
         }
+        res_g[x] = atomicAdd(&counts[cbase + bin], 8u);       // the next sector, looked at one chunk later
+        res_m |= 1u << x;
+        const uint32_t nf = n >> 3;
+        if (nf > 1u) {                                        // more than two sectors' worth arrived at once (sorted input)
+          const uint32_t g2 = atomicAdd(&counts[cbase + bin], (nf - 1u) * 8u);
+          dst[bin] = (g2 + (nf - 1u) * 8u <= b_cap[x]) ? b_off[x] + g2 - 8u : kBinFull;   // rank r >= 8 goes to dst + r
+        }
+        nfull[bin] = uint16_t(nf);
+        cnt[bin] = n & 7u;            // entries ranked >= 8 * nfull move to the buffer's front in phase B2
       }
     }
     __syncthreads();
