@@ -22,6 +22,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace tpcclus {
 
@@ -871,6 +872,39 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   const uint32_t sub = lane & 3u;                                      // four lanes per peak: lane frame R_sub
   const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
 
+  // s_misc[21 + 2b], [22 + 2b]: next group / groups done of the item in window buffer b; [25 + b]: the item
+  // (sequence number) the back warps have opened in buffer b — front warps that find their next buffer
+  // still busy help with that item instead of idling (dense tiles hand over many items per tile)
+  if (tid < 2u) s_misc[25u + tid] = 0xFFFFFFFFu;
+  // S3..S5 for the item in window buffer b: groups of 8 peaks, four lanes per peak, taken from a shared counter
+  // (shared == false: only the back warps work on the item, groups dealt statically, no bookkeeping)
+  auto assemble_item = [&](uint32_t b, auto shared_c, uint32_t bw) {
+    constexpr bool shared = decltype(shared_c)::value;
+    const uint32_t* m = wmeta + 8u * b;
+    const uint32_t npass = m[3], sector_row = m[4], npads = m[5];
+    const int32_t t_row0 = int32_t(m[6]);
+    const uint4* wb = wins + b * uint32_t(kListCap * kWinWords / 4);
+    uint4* stg = stage + b * (2u * kListCap);
+    for (uint32_t g = bw;; g += uint32_t(kBackThreads / 32)) {
+      if (shared) {
+        if (lane == 0) g = atomicAdd(&s_misc[21u + 2u * b], 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
+      }
+      if (g * 8u >= npass) break;
+      const uint32_t i = g * 8u + (lane >> 2);
+      uint4 lo4, hi4;
+      assemble4(wb + min(i, npass - 1u) * uint32_t(kWinWords / 4), nbr_tab, wtab, sub, rot_cs, rot_sn, sector_row,
+                npads, t_row0, P.tf_time_bins, lo4, hi4);
+      if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
+      if (shared) {
+        __threadfence_block();
+        __syncwarp();
+        if (lane == 0) atomicAdd(&s_misc[22u + 2u * b], 1u);
+      }
+    }
+  };
+  __syncthreads();
+
   if (warp == uint32_t(kWorkThreads / 32)) {
     // ================= committer warp: S6 look-back, S5 finish, copy-out =================
     uint32_t excl = 0;
@@ -903,7 +937,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
 
   if (warp >= uint32_t(kFrontThreads / 32)) {
     // ================= back warps: S3..S5 from the windows =================
-    const uint32_t bw = warp - uint32_t(kFrontThreads / 32);            // 0..3
     const uint32_t btid = tid - uint32_t(kFrontThreads);
     for (uint32_t q = 0;; ++q) {
       const uint32_t b = q & 1u;
@@ -921,16 +954,13 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         bar_arrive_named(kBarFull + int(b), kBackThreads + 32);
         break;
       }
-      const uint32_t npass = m[3], sector_row = m[4], npads = m[5];
-      const int32_t t_row0 = int32_t(m[6]);
-      const uint4* wb = wins + b * uint32_t(kListCap * kWinWords / 4);
-      uint4* stg = stage + b * (2u * kListCap);
-      for (uint32_t g = bw; g * 8u < npass; g += uint32_t(kBackThreads / 32)) {
-        const uint32_t i = g * 8u + (lane >> 2);
-        uint4 lo4, hi4;
-        assemble4(wb + min(i, npass - 1u) * uint32_t(kWinWords / 4), nbr_tab, wtab, sub, rot_cs, rot_sn, sector_row,
-                  npads, t_row0, P.tf_time_bins, lo4, hi4);
-        if (i < npass && sub < 2u) stg[2u * i + sub] = sub ? hi4 : lo4;
+      const bool shared = m[7] != 0u;                                   // a dense tile: front warps may help
+      if (shared && btid == 0) *reinterpret_cast<volatile uint32_t*>(&s_misc[25u + b]) = q;   // open (staging[b] is ours)
+      if (shared) assemble_item(b, std::true_type{}, 0u);
+      else assemble_item(b, std::false_type{}, warp - uint32_t(kFrontThreads / 32));
+      if (shared) {                                                     // groups taken by helpers may still be in flight
+        const uint32_t ng = (m[3] + 7u) >> 3;
+        while (*reinterpret_cast<volatile uint32_t*>(&s_misc[22u + 2u * b]) < ng) {}
       }
       bar_arrive_named(kBarWinEmpty + int(b), kWorkThreads);            // the windows are consumed
       bar_arrive_named(kBarFull + int(b), kBackThreads + 32);           // the records are staged
@@ -1071,10 +1101,20 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     uint32_t done = 0;
     do {
       const uint32_t b = q & 1u;
-      if (q >= 2u) bar_sync_named(kBarWinEmpty + int(b), kFrontThreads + kBackThreads);   // the back warps are done with buffer b
+      if (q >= 2u) {
+        // buffer b still holds item q-2: if it belongs to a dense tile, help the back warps once they have
+        // opened it; then wait for its release
+        if (wmeta[8u * b + 7u]) {
+          while (*reinterpret_cast<volatile uint32_t*>(&s_misc[25u + b]) != q - 2u) __nanosleep(100);
+          assemble_item(b, std::true_type{}, 0u);
+        }
+        bar_sync_named(kBarWinEmpty + int(b), kFrontThreads + kBackThreads);
+      }
       const uint32_t npass = min(total - done, uint32_t(kListCap));
       if (tid == 0) {
         s_misc[20] = 0u;
+        s_misc[21u + 2u * b] = 0u;
+        s_misc[22u + 2u * b] = 0u;
         uint32_t* m = wmeta + 8u * b;
         m[0] = t;
         m[1] = total;
@@ -1083,6 +1123,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
         m[4] = sector | (row << 8);
         m[5] = ri.npads;
         m[6] = uint32_t(t0 - kReach);                                   // global time of map row 0
+        m[7] = total > 3u * uint32_t(kListCap) ? 1u : 0u;               // dense tile: its items are shared with helpers
       }
       bar_sync_named(kBarWork, kFrontThreads);                          // rowoff and the group counter are ready
       // groups of 8 peaks, four lanes per peak, taken dynamically by the front warps
