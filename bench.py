@@ -316,9 +316,26 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["ms_per_launch"])
     traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(dom) \
         if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else None
+    # secondary, SM-side ceiling: both kernels are bound by instruction issue, not by HBM.
+    # Warp instructions per launch come from the same ncu capture as `traffic` (they scale with the digits
+    # of a launch); the peak is 4 schedulers x SMs x the SM clock sampled under load.
+    issue = None
+    tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))) \
+        if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else {}
+    if "warp_inst_per_digit" in tj and clk.get("sm_mhz"):
+        import torch
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        peak_issue = 4.0 * n_sm * clk["sm_mhz"] * 1e6
+        issue = {}
+        for k in ("k_bin", "k_tile"):
+            wi = tj["warp_inst_per_digit"].get(k)
+            if wi and kern[k]["ms_per_launch"] > 0:
+                ach = wi * n_dig / nfr / (kern[k]["ms_per_launch"] * 1e-3)
+                issue[k] = dict(warp_inst_per_launch=wi * n_dig / nfr, achieved=ach, peak=peak_issue,
+                                unit="warp-inst/s", frac=ach / peak_issue)
     roofline = dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
                     frac=kern[dom]["achieved_gbs"] / peak, traffic=traffic, peak_source=peak_src,
-                    kernels=kern,
+                    kernels=kern, issue=issue,
                     whole_step=dict(
                         b_min_bytes=8.0 * n_dig + 32.0 * n_cl,
                         frac_b_min=(8.0 * n_dig + 32.0 * n_cl) / (ms_step_local * 1e-3) / 1e9 / peak,
