@@ -118,9 +118,11 @@ typedef struct {
 
 typedef struct tpcclus_ctx tpcclus_ctx; /* opaque; owns all device scratch */
 
-/* Create a context on CUDA device `cuda_device`.  Allocates the charge map
- * (n_sectors x sum(pitch(npads)) x (max_core_bins + 2*halo_bins) uint16), the per-(sector,row)
- * TMA descriptors, tile-scan state and a pinned status block.
+/* Create a context on CUDA device `cuda_device`.  Allocates, once, everything a run needs
+ * (memory is reused across steps): the digit bins (one fixed-capacity list of
+ * packed 4-byte entries per sector, row and 256 time bins of the largest fragment; ~5/4 slots
+ * per cell of the bin's window), the bin counters, the tile look-back state and a pinned
+ * status block.  The charge map itself only ever exists in shared memory.
  * Errors: ERR_INVALID (null), ERR_GEOMETRY, ERR_NOMEM, ERR_CUDA (no device / wrong arch). */
 int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out);
 
@@ -140,7 +142,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
  *                     Record k is the k-th peak in ascending (sector,row,time,pad) (D10).
  * At most one digit per cell is a precondition (D2); the result for duplicate cells is
  * unspecified but memory-safe.  Up to TPCCLUS_MAX_PENDING runs may be enqueued before their
- * results are collected, all on the SAME stream (they share the charge map and execute in
+ * results are collected, all on the SAME stream (they share the digit bins and execute in
  * order; no host synchronisation is needed between the fragments of a time frame).
  * Errors (immediate): ERR_INVALID (also: too many pending runs, or a different stream while
  * runs are pending), ERR_CUDA.  Deferred to tpcclus_result: ERR_CAPACITY,
@@ -183,7 +185,7 @@ int tpcclus_get_profile(const tpcclus_ctx* ctx, double kernel_ms[TPCCLUS_N_KERNE
 /* Number of kernel launches this context has issued so far (for bench.py's gpu_launches). */
 uint64_t tpcclus_launch_count(const tpcclus_ctx* ctx);
 
-/* Bytes of device memory the context owns (charge map + scratch + staging). */
+/* Bytes of device memory the context owns (digit bins + scratch + host-staging buffers). */
 uint64_t tpcclus_device_bytes(const tpcclus_ctx* ctx);
 
 /* Free everything.  NULL is allowed. */
