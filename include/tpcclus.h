@@ -59,7 +59,7 @@ extern "C" {
                                              (2 x max_digits digits + 2 x max_clusters records) */
 
 #define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
-#define TPCCLUS_MAX_NPADS  246u  /* 8 + npads + 2 columns must fit a 256-wide TMA box */
+#define TPCCLUS_MAX_NPADS  256u  /* the pad of a digit is a uint8 */
 #define TPCCLUS_MAX_PENDING 64    /* runs that may be enqueued before their tpcclus_result */
 #define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
 

@@ -318,3 +318,73 @@ def test_direct_binning_fallback_matches(monkeypatch):
     monkeypatch.setenv("TPCCLUS_BIN_DIRECT", "1")
     b, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
     assert len(a) > 1e4 and a.tobytes() == b.tobytes()
+
+
+def _random_cells(rng, n_sectors, npads, t_lo, t_hi, n, max_q=400.0):
+    """n random distinct cells with charges on the 1/16 ADC grid (some saturated, some tied)."""
+    cells = {}
+    rows = len(npads)
+    while len(cells) < n:
+        s = int(rng.integers(n_sectors)); r = int(rng.integers(rows))
+        p = int(rng.integers(npads[r])); t = int(rng.integers(t_lo, t_hi))
+        q = float(rng.integers(32, int(max_q * 16))) / 16.0
+        if rng.random() < 0.05:
+            q = 1023.0
+        if rng.random() < 0.2:
+            q = 20.0                               # exact ties
+        cells[(s, r, p, t)] = q
+    return [(s, r, p, t, q) for (s, r, p, t), q in cells.items()]
+
+
+def test_maximum_geometry():
+    """Largest geometry the ABI accepts: 256 rows of up to 256 pads (a 1-pad row too), a 65536-bin time
+    frame, fragments at its very end and with the largest halo-free core (one CTA per SM: the 266 x 264
+    charge map takes most of the shared memory).  Dense random blobs so that peaks touch, split and saturate."""
+    rng = np.random.default_rng(11)
+    npads = [256] * 256
+    npads[3] = 1
+    npads[200] = 17
+    # blobs of cells around random centres (clusters of touching cells)
+    cells = {}
+    for _ in range(900):
+        s = int(rng.integers(2)); r = int(rng.choice([0, 3, 77, 200, 255]))
+        pc = int(rng.integers(npads[r])); tc = int(rng.integers(65536 - 700, 65536))
+        for _ in range(12):
+            p = pc + int(rng.integers(-2, 3)); t = tc + int(rng.integers(-3, 4))
+            if 0 <= p < npads[r] and 65536 - 700 <= t < 65536:
+                q = 1023.0 if rng.random() < 0.03 else float(rng.integers(32, 4000)) / 16.0
+                cells[(s, r, p, t)] = q
+    d, offs = digits_from_cells([(s, r, p, t, q) for (s, r, p, t), q in cells.items()], n_sectors=2)
+    dd = to_device_digits(d)
+    for core, halo, spans in [(300, 8, [(65236, 65536), (64936, 65236)]), (700, 0, [(64836, 65536)])]:
+        with GpuClusterizer(npads, n_sectors=2, tf_time_bins=65536, max_core_bins=core, halo_bins=halo,
+                            max_digits=len(d)) as g:
+            for b, e in spans:
+                got, st = g.run(dd, offs, b, e)
+                ref, ost = oracle.run(d, offs, npads, n_sectors=2, tf_time_bins=65536, t_core_begin=b,
+                                      t_core_end=e, halo_bins=halo)
+                assert st["n_digits_dropped"] == ost["n_digits_dropped"]
+                assert len(ref) > 100
+                assert_clusters_match(got, ref, f"max geometry core {core} [{b},{e})")
+                assert got.tobytes() == ref.tobytes()
+
+
+def test_duplicate_cells_are_memory_safe_and_context_survives():
+    """D2's precondition (one digit per cell) violated massively: the result is unspecified, but the
+    library must neither fault nor leave the context unusable (bins are bounded; overfull bins drop)."""
+    npads = [8, 8]
+    n = 200_000
+    d = np.zeros(n, dtype=oracle.DIGIT_DTYPE)
+    d["row"] = 1
+    d["pad"] = 3
+    d["time"] = 7
+    d["charge"] = 10.0
+    offs = np.array([0, n], dtype=np.uint64)
+    good_cells = [(0, 0, 2, 5, 9.0), (0, 0, 3, 5, 30.0), (0, 1, 4, 20, 12.0)]
+    dg, og = digits_from_cells(good_cells, n_sectors=1)
+    with GpuClusterizer(npads, n_sectors=1, tf_time_bins=64, max_digits=n) as g:
+        _, st = g.run(to_device_digits(d), offs, 0, 64, capacity=16, check=False)
+        assert st["cuda_error"] == 0
+        got, st = g.run(to_device_digits(dg), og, 0, 64)
+        ref, _ = oracle.run(dg, og, npads, n_sectors=1, tf_time_bins=64)
+        assert st["status"] == 0 and got.tobytes() == ref.tobytes() and len(ref) == 2
