@@ -388,3 +388,25 @@ def test_duplicate_cells_are_memory_safe_and_context_survives():
         got, st = g.run(to_device_digits(dg), og, 0, 64)
         ref, _ = oracle.run(dg, og, npads, n_sectors=1, tf_time_bins=64)
         assert st["status"] == 0 and got.tobytes() == ref.tobytes() and len(ref) == 2
+
+
+def test_many_small_sectors():
+    """200 sectors (more than k_bin has CTAs) of uneven, partly empty digit slices: CTAs cross sector
+    boundaries between chunks (buffer flush + re-reservation per sector), 16-byte pairs straddle slices."""
+    rng = np.random.default_rng(23)
+    npads = [20, 33, 7]
+    n_sectors = 200
+    cells = {}
+    for s in range(n_sectors):
+        if s % 7 == 3:
+            continue                                     # empty slice
+        for _ in range(int(rng.integers(1, 60))):
+            r = int(rng.integers(3)); pc = int(rng.integers(npads[r])); tc = int(rng.integers(0, 300))
+            for _ in range(6):
+                p = pc + int(rng.integers(-1, 2)); t = tc + int(rng.integers(-2, 3))
+                if 0 <= p < npads[r] and 0 <= t < 300:
+                    cells[(s, r, p, t)] = float(rng.integers(32, 3000)) / 16.0
+    d, offs = digits_from_cells([(s, r, p, t, q) for (s, r, p, t), q in cells.items()], n_sectors=n_sectors)
+    got, ref, st = both(d, offs, npads, n_sectors=n_sectors, tf_time_bins=300)
+    assert len(ref) > 2000 and st["n_digits_dropped"] == 0
+    assert got.tobytes() == ref.tobytes()
