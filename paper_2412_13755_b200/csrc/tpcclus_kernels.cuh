@@ -1,19 +1,20 @@
 // tpcclus_kernels.cuh — sm_100a kernels of the TPC cluster finder (device side).
 //
 // Steps of SURVEY.md §8(a) and where they run:
-//   S0  set-up               k_init   zero the per-tile digit counters and the run status
-//   S1  charge-map fill      k_bin    16-byte digit loads, D1 quantisation, digit -> packed 4-byte
-//                                     record appended to the list of every (sector,row,time-tile)
-//                                     whose window holds it (tile halo duplicated here)
-//                            k_tile   the tile's list is staged in shared memory by a TMA bulk copy
-//                                     and scattered into the (pad x time) charge map of the tile,
-//                                     which lives in shared memory only
-//   S2  peak finding         k_tile   digit-driven 3x3 ordered-maximum test on the smem map -> flag bitmap
-//   S3  peak count S(c)      k_tile   9x9 flag window from the smem flag bitmap
-//   S4  5x5 assembly         k_tile   one thread per peak, charges from the smem map
-//   S5  centroid / width     k_tile   exact integer moments, fp64 finish
-//   S6  ordered compaction   k_tile   popc prefix inside the tile + decoupled look-back across tiles
-//                                     in (sector,row,time) ticket order, by a dedicated warp
+//   S0  set-up               k_init   zero the per-bin entry counters and the run status
+//   S1  charge-map fill      k_bin    TMA-staged digit chunks (16-byte pairs), D1 quantisation, digit ->
+//                                     packed 4-byte entry in the list of every (sector,row,256-bin) digit
+//                                     bin whose window holds it; write-combined: one 32-byte sector and
+//                                     one global atomic per 8 entries
+//                            k_tile   front warps: the bin's list is scattered into the (pad x time)
+//                                     charge map of the tile, which lives in shared memory only
+//   S2  peak finding         k_tile   front warps: digit-driven 3x3 ordered-maximum test on the smem map
+//                                     -> flag bitmap; then each peak's 80-byte window is cut out
+//   S3  peak count S(c)      k_tile   back warps: other peaks of the 9x9 flag window, table-driven
+//   S4  5x5 assembly         k_tile   back warps: four lanes per peak (rotation classes)
+//   S5  centroid / width     k_tile   back warps: exact integer moments; committer warp: fp64 finish
+//   S6  ordered compaction   k_tile   front warps: popc prefix inside the tile; committer warp: decoupled
+//                                     look-back across tiles in (sector,row,time) ticket order, copy-out
 //   S7  fragment ownership   k_tile   tiles cover exactly the core [b,e); halo rows never emit
 //
 // Definitions D1..D12 are those of SURVEY.md §8(c) (restated in DESIGN.md §2); the D-number
@@ -616,7 +617,7 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
     if (lane == 0) st_release_u64(state, pack_state(epoch, kStPrefix, aggregate));
     return 0;
   }
-  // the tile's own count (kStAgg) was published by its workers right after the count phase
+  // the tile's own count (kStAgg) was published by its front warps right after the count phase
   uint32_t sum = 0;
   int64_t look = int64_t(tile) - 1;
   while (true) {
@@ -679,7 +680,7 @@ __device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
   return e;
 }
 
-struct __align__(16) RawRec {       // what the workers stage: D7's exact integers; the committer turns it into ClusterRec
+struct __align__(16) RawRec {       // what the back warps stage: D7's exact integers; the committer turns it into ClusterRec
   uint32_t w0, time, w2;            // as in ClusterRec
   uint32_t W;                       // sum of weights, units of 1/(16*2520) ADC
   int32_t Mp, Mt;                   // sum w dp, sum w dt
