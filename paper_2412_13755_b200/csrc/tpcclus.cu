@@ -219,7 +219,10 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
       cudaMemset(c->d_status, 0, sizeof(DevStatus)) != cudaSuccess)
     return fail(TPCCLUS_ERR_CUDA);
 
-  if (cudaFuncSetAttribute(k_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, int(c->smem_bytes)) != cudaSuccess)
+  // the attribute belongs to the function, not to this context: always allow the device maximum so that
+  // contexts with different geometries can coexist
+  if (c->smem_bytes > uint32_t(prop.sharedMemPerBlockOptin)) return fail(TPCCLUS_ERR_GEOMETRY);
+  if (cudaFuncSetAttribute(k_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, int(prop.sharedMemPerBlockOptin)) != cudaSuccess)
     return fail(TPCCLUS_ERR_CUDA);
   int occ = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tile, kThreads, c->smem_bytes) != cudaSuccess || occ < 1)
@@ -230,7 +233,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     c->bin_aggregated = nb_max <= kBinMaxNb && bin_smem_bytes(nb_max) <= uint32_t(prop.sharedMemPerBlockOptin) &&
                         !std::getenv("TPCCLUS_BIN_DIRECT");
     if (c->bin_aggregated &&
-        cudaFuncSetAttribute(k_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bin_smem_bytes(nb_max))) != cudaSuccess)
+        cudaFuncSetAttribute(k_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, int(prop.sharedMemPerBlockOptin)) != cudaSuccess)
       return fail(TPCCLUS_ERR_CUDA);
     if (c->bin_aggregated) {
       int bocc = 0;

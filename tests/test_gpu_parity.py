@@ -410,3 +410,23 @@ def test_many_small_sectors():
     got, ref, st = both(d, offs, npads, n_sectors=n_sectors, tf_time_bins=300)
     assert len(ref) > 2000 and st["n_digits_dropped"] == 0
     assert got.tobytes() == ref.tobytes()
+
+
+def test_two_contexts_with_different_geometries_coexist():
+    """Shared-memory limits are per kernel function, not per context: a small context created after a
+    large one must not break the large one (and vice versa)."""
+    rng = np.random.default_rng(3)
+    big_np, small_np = [256, 200], [12]
+    cb = _random_cells(rng, 1, big_np, 0, 120, 1500)
+    cs = _random_cells(rng, 1, small_np, 0, 50, 200)
+    db, ob = digits_from_cells(cb, n_sectors=1)
+    ds, os_ = digits_from_cells(cs, n_sectors=1)
+    with GpuClusterizer(big_np, n_sectors=1, tf_time_bins=120, max_digits=len(db)) as gb:
+        with GpuClusterizer(small_np, n_sectors=1, tf_time_bins=50, max_digits=len(ds)) as gs:
+            got_b, _ = gb.run(to_device_digits(db), ob, 0, 120)
+            got_s, _ = gs.run(to_device_digits(ds), os_, 0, 50)
+            got_b2, _ = gb.run(to_device_digits(db), ob, 0, 120)
+    ref_b, _ = oracle.run(db, ob, big_np, n_sectors=1, tf_time_bins=120)
+    ref_s, _ = oracle.run(ds, os_, small_np, n_sectors=1, tf_time_bins=50)
+    assert got_b.tobytes() == ref_b.tobytes() == got_b2.tobytes() and len(ref_b) > 50
+    assert got_s.tobytes() == ref_s.tobytes() and len(ref_s) > 5
