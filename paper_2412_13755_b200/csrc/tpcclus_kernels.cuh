@@ -37,7 +37,7 @@ constexpr int      kBinShift     = 8;
 constexpr int      kBinBoxH      = kBinT + 2 * kReach;    // time rows a bin's window spans (266)
 static_assert((1 << kBinShift) == kBinT && kBinT == kTileT, "a digit bin is one tile");
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
-constexpr int      kListCap      = 96;    // peaks per hand-over item (capacity of one window / staging buffer)
+constexpr int      kListCap      = 120;   // peaks per hand-over item (capacity of one window / staging buffer)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 
