@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(CSRC, "libtpcclus.so")
 SOURCES = ["tpcclus.cu"]
-DEPS = ["tpcclus.cu", "tpcclus_kernels.cuh", os.path.join("..", "..", "include", "tpcclus.h")]
+DEPS = ["tpcclus.cu", "tpcclus_kernels.cuh", "tpcclus_tile.cuh", os.path.join("..", "..", "include", "tpcclus.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -31,7 +31,7 @@ struct tpcclus_ctx {
   uint32_t max_bins = 0;
   uint64_t sec_list_elems = 0;    // digit-list elements per sector
   uint32_t max_tiles = 0;
-  uint32_t map_bytes_max = 0, bm_words = 0, smem_bytes = 0;
+  uint32_t map_bytes_max = 0, smem_bytes = 0;
   int tile_grid = 0;              // persistent grid of k_tile
   int bin_ctas_per_sm = 1;        // resident k_bin CTAs per SM (occupancy query)
   bool bin_aggregated = false;    // k_bin (CTA-aggregated) usable for this geometry, else k_bin_direct
@@ -192,14 +192,14 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     max_npads = std::max<uint32_t>(max_npads, ri.npads);
   }
   c->sec_list_elems = off;
-  c->bm_words = (max_npads + 8 + 31) / 32 + 1;
-  c->map_bytes_max = roundup(uint32_t(kBoxH) * max_W * 2u + uint32_t(kBoxH) * c->bm_words * 4u, 16);
+  (void)max_npads;
+  c->map_bytes_max = roundup(uint32_t(kBoxH) * max_W * 2u + uint32_t(kBoxH) * flag_pitch_bytes(max_W), 16) + 16u;
   const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * c->tiles_per_row_max;
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = c->map_bytes_max + 2 * kListCap * kWinWords * 4 + 2 * kListCap * 32 + 16 + 32 * 4 + 2 * 4 * 4 + 2 * 8 * 4 +
-                  (kTileT + 4) * 4 + kNbrTabWords * 4 + 12 * 4 + 128;
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kWorkWarps * kWarpList * 4 + 16 + 32 * 4 + 2 * 4 * 4 +
+                  kNbrTabWords * 4 + 12 * 4 + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;
@@ -362,7 +362,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     tp.theta = g.peak_min_q16;
     tp.epoch = c->epoch;
     tp.map_bytes_max = c->map_bytes_max;
-    tp.bm_words = c->bm_words;
+    tp.pad_ = 0;
     const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->tile_grid)));
     k_tile<<<grid, kThreads, c->smem_bytes, st>>>(tp);
     c->launches++;
