@@ -184,7 +184,19 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     ri.npads = c->npads[r];
     ri.W = uint16_t(roundup(ri.npads + 2 * kColOff, 8));
     ri.cap = roundup(bin_rows * ri.npads + bin_rows * ri.npads / 4 + cap_margin, 8);
-    ri.pad_ = 0;
+    ri.ns = uint16_t(ri.W / 8);
+    ri.fpb = uint16_t(flag_pitch_bytes(ri.W));
+    {
+      // sweep tasks: as many row segments as the worker threads can take at once, each flagging segL of the
+      // kBoxH - 2 rows that carry flags
+      const uint32_t rows_out = uint32_t(kBoxH) - 2u;
+      const uint32_t nseg_max = std::max<uint32_t>(uint32_t(kWorkThreads) / ri.ns, 1u);
+      const uint32_t L = (rows_out + nseg_max - 1) / nseg_max;
+      ri.segL = uint16_t(L);
+      ri.ntasks = uint16_t(ri.ns * ((rows_out + L - 1) / L));
+      ri.rcp_ns = (65536u + ri.ns - 1u) / ri.ns;
+    }
+    ri.pad_[0] = ri.pad_[1] = 0;
     if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
     ri.list_off = uint32_t(off);
     off += uint64_t(c->bins_per_row_max) * ri.cap;
@@ -193,13 +205,13 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   }
   c->sec_list_elems = off;
   (void)max_npads;
-  c->map_bytes_max = roundup(uint32_t(kBoxH) * max_W * 2u + uint32_t(kBoxH) * flag_pitch_bytes(max_W), 16) + 16u;
+  c->map_bytes_max = roundup(2u * uint32_t(kMapGuard) + uint32_t(kBoxH) * max_W * 2u + uint32_t(kBoxH) * flag_pitch_bytes(max_W), 16) + 16u;
   const uint64_t tiles = uint64_t(g->n_sectors) * g->n_rows * c->tiles_per_row_max;
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kWorkWarps * kWarpList * 4 + 16 + 32 * 4 + 2 * 4 * 4 +
-                  kNbrTabWords * 4 + 12 * 4 + 128;
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kNbrTabWords * 4 + kListCap * 4 + 16 + 32 * 4 + 2 * 4 * 4 +
+                  16 * 4 + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;
@@ -362,7 +374,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     tp.theta = g.peak_min_q16;
     tp.epoch = c->epoch;
     tp.map_bytes_max = c->map_bytes_max;
-    tp.pad_ = 0;
+    tp.theta2 = uint32_t(g.peak_min_q16) | (uint32_t(g.peak_min_q16) << 16);
     const int grid = int(std::min<uint32_t>(n_tiles, uint32_t(c->tile_grid)));
     k_tile<<<grid, kThreads, c->smem_bytes, st>>>(tp);
     c->launches++;

@@ -41,13 +41,20 @@ constexpr int      kListCap      = 256;   // records per hand-over item (capacit
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 
-struct RowInfo {              // one per pad row (device table)
+struct RowInfo {              // one per pad row (device table), 32 bytes
   uint32_t list_off;          // element offset of this row's bins inside one sector's digit lists
   uint32_t cap;               // list capacity of one bin (multiple of 8): window cells * 5/4 + padding margin
   uint16_t npads;
   uint16_t W;                 // smem map pitch in cells = roundup8(npads + 4)
-  uint32_t pad_;
+  // k_tile's sweep over a tile of this row: strips of 8 cells x row segments
+  uint16_t ns;                // strips per map row = W / 8
+  uint16_t fpb;               // flag bytes per map row = flag_pitch_bytes(W)
+  uint16_t segL;              // map rows flagged per segment
+  uint16_t ntasks;            // ns * number of segments
+  uint32_t rcp_ns;            // ceil(2^16 / ns): task / ns = (task * rcp_ns) >> 16 for task < 512 (ns <= 64)
+  uint32_t pad_[2];
 };
+static_assert(sizeof(RowInfo) == 32, "RowInfo is 32 bytes");
 
 struct DevStatus {            // device-side run status, copied to pinned host memory after the run
   unsigned long long n_dropped;
@@ -92,7 +99,7 @@ struct TileParams {
   uint32_t theta;                      // peak_min_q16
   uint32_t epoch;                      // run counter, tags tile_state words
   uint32_t map_bytes_max;              // smem bytes reserved for map + flag bytes
-  uint32_t pad_;
+  uint32_t theta2;                     // theta | theta << 16
 };
 
 // ----------------------------------------------------------------------------------------

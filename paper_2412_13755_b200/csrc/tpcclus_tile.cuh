@@ -15,8 +15,9 @@
 //             byte store, so the flag map needs neither atomics nor clearing                   (S2)
 //   count     one lane per core row: popc of its flag words, warp scan, CTA scan -> the position of every
 //             peak in (time,pad) order; the tile's count is published for the look-back       (S6, S7)
-//   build     every warp builds the clusters of ITS 16 core rows, four lanes per peak, reading charges and
-//             flags straight from the map (S3..S5); exact integer records (RawRec) go to a staging buffer
+//   list      the row owners write their peaks, in order, into the tile's peak list
+//   build     one thread per peak, dense over the list: the 25 charges and the 9x9 flag window straight from
+//             the map (S3..S5); exact integer records (RawRec) go to a staging buffer
 //   commit    the committer warp: decoupled look-back across tiles, D8 finish in fp64, ordered copy-out (S6)
 //
 // Definitions D1..D12: SURVEY.md §8(c), restated in DESIGN.md §2.  No code here is shared with oracle/.
@@ -74,42 +75,26 @@ __device__ __forceinline__ uint32_t lookback_exclusive(unsigned long long* state
   return sum;
 }
 
-// ----------------------------------------------------------------------------------------
-// S3..S5, four lanes per peak.
-//
-// The 24 cells around a peak P split into four rotation classes of six: lane `sub` (0..3) owns
-// the images under the quarter turn R_sub of the base cells
-//     I0 = (1,0)  I1 = (1,1)                      inner ring (always members when charged, D5)
-//     O0 = (2,-1) O1 = (2,0) O2 = (2,1) O3 = (2,2) outer ring (monotone descent, D5)
-// written (a,b) = (pad, time) offsets in the lane's own frame; R_s(a,b) = (a cs - b sn, a sn + b cs)
-// with (cs,sn) = (1,0),(0,1),(-1,0),(0,-1).  The inner cells 8-adjacent to O0..O3 are
-// (1,-1),(1,0),(1,1) of the same frame, so a lane reads 7 charges besides P.  Moments are summed in
-// the lane frame with constant coefficients and rotated once.  D6's S(c) comes from the OTHER peaks
-// of the 9x9 flag window: each one adds a table entry (one nibble per owned cell it is within
-// distance 2 of, plus an "is this outer cell" bit).  The four partial sums are combined with two
-// xor-shuffles; the record is staged as exact integers (RawRec) and finished by the committer warp.
-// ----------------------------------------------------------------------------------------
-constexpr int kNbrTabWords = 4 * 81;
-constexpr uint32_t kShareL = 2520u;                      // D6: lcm(1..9)
 
-// entry for lane frame s and another peak at window row k (time j-4+k), column i (pad p-4+i)
-__device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
-  const int s = int(idx / 81u), r = int(idx % 81u);
-  const int u = r % 9 - 4, v = r / 9 - 4;               // (pad, time) offset of the other peak
-  int up, vp;                                           // the same offset in the lane frame: R_s^-1 (u,v)
-  if (s == 0)      { up = u;  vp = v; }
-  else if (s == 1) { up = v;  vp = -u; }
-  else if (s == 2) { up = -u; vp = -v; }
-  else             { up = -v; vp = u; }
-  const int ca[6] = {1, 1, 2, 2, 2, 2}, cb[6] = {0, 1, -1, 0, 1, 2};
-  uint32_t e = 0;
-  for (int c = 0; c < 6; ++c) {
-    const int da = ca[c] - up, db = cb[c] - vp;
-    if (da >= -2 && da <= 2 && db >= -2 && db <= 2) e += 1u << (4 * c);
-    if (c >= 2 && da == 0 && db == 0) e |= 1u << (24 + c - 2);
-  }
-  return e;
+// ----------------------------------------------------------------------------------------
+// shared-memory access by 32-bit shared-space address (no generic-address arithmetic in the hot loops)
+// ----------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
 }
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds16(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts8(uint32_t a, uint32_t v) { asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v)); }
 
 struct __align__(16) RawRec {       // what the workers stage: D7's exact integers; the committer turns it into ClusterRec
   uint32_t w0, time, w2;            // as in ClusterRec
@@ -119,98 +104,122 @@ struct __align__(16) RawRec {       // what the workers stage: D7's exact intege
 };
 static_assert(sizeof(RawRec) == 32, "raw record is 32 bytes");
 
+// ----------------------------------------------------------------------------------------
+// S3..S5, one thread per peak.
+//
+// The 25 cells of the 5x5 window are numbered k = 5 (dt+2) + (dp+2).  D6's S(c) comes from the OTHER peaks of
+// the 9x9 flag window around P: each adds a table entry — one nibble per window cell it is within Chebyshev
+// distance 2 of (25 nibbles = 4 words) — so S(c) - 1 is the cell's nibble of the sum.  Column and row sums of
+// the weights give D7's moments with constant coefficients.
+// ----------------------------------------------------------------------------------------
+constexpr int kNbrTabWords = 81 * 4;
+constexpr uint32_t kShareL = 2520u;                      // D6: lcm(1..9)
+
+// word `idx & 3` of the entry for another peak at window row v+4 (time offset v), column u+4 (pad offset u)
+__device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
+  const int r = int(idx >> 2), word = int(idx & 3u);
+  const int u = r % 9 - 4, v = r / 9 - 4;
+  uint32_t e = 0;
+  for (int n = 0; n < 8; ++n) {
+    const int k = word * 8 + n;
+    if (k >= 25) break;
+    const int dt = k / 5 - 2, dp = k % 5 - 2;
+    if (dp - u >= -2 && dp - u <= 2 && dt - v >= -2 && dt - v <= 2) e |= 1u << (4 * n);
+  }
+  return e;
+}
+
 // Flag bytes of a tile: row j of the map has a 4-byte zero prefix followed by one byte per strip of 8 map
 // columns (bit b of byte s <-> column 8 s + b), padded with zero bytes to a multiple of 4.  Read as 32-bit
 // words, the flag of pad p sits at bit index 32 + kColOff + p of the row; the zero prefix makes the 9-bit
 // window that starts four pads to the left of a peak addressable without a branch for p < 4.
 __host__ __device__ inline uint32_t flag_pitch_bytes(uint32_t W) { return 4u + (((W >> 3) + 3u) & ~3u); }
 
-// All 32 lanes call this; lanes 4g..4g+3 build the cluster of the peak at map row j, pad `pad`, from the
-// tile's map and flag bytes.  Returns the two 16-byte halves of the RawRec in every lane of the group.
-__device__ __forceinline__ void build4(const uint16_t* __restrict__ map, const uint32_t* __restrict__ fw, uint32_t W,
-                                       uint32_t nfw, uint32_t j, uint32_t pad, const uint32_t* __restrict__ nbr_tab,
-                                       const uint32_t* __restrict__ wtab, uint32_t sub, int32_t cs, int32_t sn,
-                                       uint32_t sector_row /* sector | row << 8 */, uint32_t npads, int32_t t_row0,
-                                       uint32_t tf_time_bins, uint4& lo, uint4& hi) {
-  // ---- charges: P and the seven cells of this lane's rotation class ----
-  const uint16_t* c = map + j * W + (pad + kColOff);
-  const int32_t X = sn * int32_t(W) + cs, Y = cs * int32_t(W) - sn;     // steps of (a,b) in map cells
-  const uint32_t qP = c[0];
-  const uint32_t qIm = c[X - Y], qI0 = c[X], qI1 = c[X + Y];
-  const uint32_t qO0 = c[2 * X - Y], qO1 = c[2 * X], qO2 = c[2 * X + Y], qO3 = c[2 * X + 2 * Y];
-  // ---- the 9x9 flag window around P, three rows per word: bit 9*(k%3)+i of G[k/3] <-> row j-4+k, pad
-  //      p-4+i.  Lane s reads rows s and s+4, lane 0 also row 8; OR-combined over the four lanes ----
-  uint32_t G0 = 0, G1 = 0, G2 = 0;
+// Build the cluster of the peak at map row j, pad `pad` (one thread).  map_s / flag_s / tab_s / wtab_s are
+// shared-space addresses of the tile's map, its flag bytes, the neighbour table and the L/S table.
+__device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t pitch /* 2 W */, uint32_t fpb, uint32_t j,
+                                       uint32_t pad, uint32_t tab_s, uint32_t wtab_s, uint32_t sector_row, uint32_t npads,
+                                       int32_t t_row0, uint32_t tf_time_bins, uint4& lo, uint4& hi) {
+  // ---- the 25 charges ----
+  uint32_t q[25];
   {
-    const uint32_t b0 = pad + (32u + uint32_t(kColOff) - 4u);           // bit index of pad p-4
-    const uint32_t sh = b0 & 31u;
-    const uint32_t* rowp = fw + (j - 4u) * nfw + (b0 >> 5);
-    auto row_bits = [&](uint32_t k) -> uint32_t {
-      return __funnelshift_r(rowp[k * nfw], rowp[k * nfw + 1], sh) & 0x1FFu;
-    };
-    const uint32_t fa = row_bits(sub), fb = row_bits(sub + 4u), fc = sub == 0u ? row_bits(8u) : 0u;
-    // row k -> word k/3, shift 9*(k%3)
-    if (sub < 3u) G0 = fa << (9u * sub); else G1 = fa;                   // rows 0,1,2 | 3
-    if (sub < 2u) G1 |= fb << (9u * (sub + 1u)); else G2 = fb << (9u * (sub - 2u));   // rows 4,5 | 6,7
-    G2 |= fc << 18;                                                      // row 8
+    const uint32_t base = map_s + j * pitch + 2u * (pad + uint32_t(kColOff));
 #pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
-      G0 |= __shfl_xor_sync(0xffffffffu, G0, o);
-      G1 |= __shfl_xor_sync(0xffffffffu, G1, o);
-      G2 |= __shfl_xor_sync(0xffffffffu, G2, o);
+    for (int dt = -2; dt <= 2; ++dt) {
+      const uint32_t rb = base + uint32_t(dt) * pitch;
+#pragma unroll
+      for (int dp = -2; dp <= 2; ++dp) q[(dt + 2) * 5 + dp + 2] = lds16(rb + uint32_t(2 * dp));
     }
-    G1 &= ~(1u << 13);                                                  // P itself (row 4, column 4)
   }
-  const int32_t tglob = t_row0 + int32_t(j);                            // t_row0 = global time of map row 0
-  uint32_t acc = 0;                                                     // nibble c: other peaks within distance 2 of cell c
+  // ---- the 9x9 flag window: R[k] = flags of row j-4+k, bit i <-> pad p-4+i ----
+  uint32_t R[9];
   {
-    const uint32_t* t = nbr_tab + sub * 81u;
-    while (G0) { const uint32_t b = __ffs(G0) - 1; G0 &= G0 - 1; acc += t[b]; }
-    while (G1) { const uint32_t b = __ffs(G1) - 1; G1 &= G1 - 1; acc += t[27 + b]; }
-    while (G2) { const uint32_t b = __ffs(G2) - 1; G2 &= G2 - 1; acc += t[54 + b]; }
-  }
-  // D5 membership
-  const bool mI0 = qI0 != 0u, mI1 = qI1 != 0u;
-  const bool mO0 = qO0 != 0u && !((acc >> 24) & 1u) && (qIm >= qO0 || qI0 >= qO0);
-  const bool mO1 = qO1 != 0u && !((acc >> 25) & 1u) && (qIm >= qO1 || qI0 >= qO1 || qI1 >= qO1);
-  const bool mO2 = qO2 != 0u && !((acc >> 26) & 1u) && (qI0 >= qO2 || qI1 >= qO2);
-  const bool mO3 = qO3 != 0u && !((acc >> 27) & 1u) && (qI1 >= qO3);
-  // D6 weights w = Q * L / S, S = 1 + other peaks within distance 2
-  uint32_t meta = 0;                                                    // ncells | n_saturated << 8 | n_split << 16
-  auto weight = [&](bool m, uint32_t q, uint32_t nib) -> uint32_t {
-    const uint32_t S = (acc >> (4 * nib)) & 15u;                        // S - 1
-    if (m) meta += 1u + (q == kQClamp ? 0x100u : 0u) + (S ? 0x10000u : 0u);
-    return m ? q * wtab[S] : 0u;
-  };
-  const uint32_t wI0 = weight(mI0, qI0, 0), wI1 = weight(mI1, qI1, 1);
-  const uint32_t wO0 = weight(mO0, qO0, 2), wO1 = weight(mO1, qO1, 3);
-  const uint32_t wO2 = weight(mO2, qO2, 4), wO3 = weight(mO3, qO3, 5);
-  // D7 moments in the lane frame, then rotated (cs*sn = 0)
-  const uint32_t wO = wO0 + wO1 + wO2 + wO3, wI = wI0 + wI1;
-  uint32_t Wsum = wI + wO;
-  const int32_t Ma = int32_t(wI + 2u * wO);
-  const int32_t Mb = int32_t(wI1 + wO2 + 2u * wO3) - int32_t(wO0);
-  const uint32_t Maa = wI + 4u * wO;
-  const uint32_t Mbb = wI1 + wO0 + wO2 + 4u * wO3;
-  int32_t Mp = cs * Ma - sn * Mb, Mt = sn * Ma + cs * Mb;
-  uint32_t Mpp = cs ? Maa : Mbb, Mtt = cs ? Mbb : Maa;
+    const uint32_t b0 = pad + (32u + uint32_t(kColOff) - 4u);           // bit index of pad p-4 inside a flag row
+    const uint32_t sh = b0 & 31u;
+    const uint32_t a0 = flag_s + (j - 4u) * fpb + 4u * (b0 >> 5);
 #pragma unroll
-  for (int o = 1; o <= 2; o <<= 1) {
-    Wsum += __shfl_xor_sync(0xffffffffu, Wsum, o);
-    Mp += __shfl_xor_sync(0xffffffffu, Mp, o);
-    Mt += __shfl_xor_sync(0xffffffffu, Mt, o);
-    Mpp += __shfl_xor_sync(0xffffffffu, Mpp, o);
-    Mtt += __shfl_xor_sync(0xffffffffu, Mtt, o);
-    meta += __shfl_xor_sync(0xffffffffu, meta, o);
+    for (int k = 0; k < 9; ++k) R[k] = __funnelshift_r(lds32(a0 + uint32_t(k) * fpb), lds32(a0 + uint32_t(k) * fpb + 4u), sh) & 0x1FFu;
+    R[4] &= ~(1u << 4);                                                  // P itself
   }
-  Wsum += qP * kShareL;                                                 // D6: w(P) = L Q(P)
+  // ---- D6: other peaks of the window -> S(c) - 1 per cell (nibbles) ----
+  uint32_t acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;
+  {
+    uint32_t G0 = R[0] | (R[1] << 9) | (R[2] << 18), G1 = R[3] | (R[4] << 9) | (R[5] << 18), G2 = R[6] | (R[7] << 9) | (R[8] << 18);
+    auto add = [&](uint32_t b) {
+      const uint4 e = lds128(tab_s + 16u * b);
+      acc0 += e.x; acc1 += e.y; acc2 += e.z; acc3 += e.w;
+    };
+    while (G0) { const uint32_t b = __ffs(G0) - 1; G0 &= G0 - 1; add(b); }
+    while (G1) { const uint32_t b = __ffs(G1) - 1; G1 &= G1 - 1; add(27u + b); }
+    while (G2) { const uint32_t b = __ffs(G2) - 1; G2 &= G2 - 1; add(54u + b); }
+  }
+  const uint32_t qP = q[12];
+  uint32_t col[5] = {0u, 0u, 0u, 0u, 0u}, rowsum[5] = {0u, 0u, 0u, 0u, 0u};
+  uint32_t ncells = 1u, nsat = (qP == kQClamp) ? 1u : 0u, nsplit = 0u;
+#pragma unroll
+  for (int k = 0; k < 25; ++k) {
+    if (k == 12) continue;
+    const int dt = k / 5 - 2, dp = k % 5 - 2;
+    const uint32_t qc = q[k];
+    // D5: has charge, is not a peak; outer ring: some 8-adjacent inner-ring cell has Q >= Q(c)
+    bool m = qc != 0u && !((R[dt + 4] >> (dp + 4)) & 1u);
+    if (dt == -2 || dt == 2 || dp == -2 || dp == 2) {
+      uint32_t best = 0u;
+#pragma unroll
+      for (int it = -1; it <= 1; ++it)
+#pragma unroll
+        for (int ip = -1; ip <= 1; ++ip) {
+          if (ip == 0 && it == 0) continue;
+          if (ip - dp > 1 || dp - ip > 1 || it - dt > 1 || dt - it > 1) continue;
+          best = max(best, q[(it + 2) * 5 + ip + 2]);
+        }
+      m = m && best >= qc;
+    }
+    // D6: w = Q * L / S
+    const uint32_t accw = (k < 8) ? acc0 : (k < 16) ? acc1 : (k < 24) ? acc2 : acc3;
+    const uint32_t nib = (accw >> (4 * (k & 7))) & 15u;                  // S - 1
+    const uint32_t w = m ? qc * lds32(wtab_s + 4u * nib) : 0u;
+    col[dp + 2] += w;
+    rowsum[dt + 2] += w;
+    if (m) {
+      ncells += 1u;
+      nsat += (qc == kQClamp) ? 1u : 0u;
+      nsplit += nib;
+    }
+  }
+  // D7 moments from the column / row sums
+  const uint32_t Wsum = col[0] + col[1] + col[2] + col[3] + col[4] + qP * kShareL;   // D6: w(P) = L Q(P)
+  const int32_t Mp = int32_t(2u * col[4] + col[3]) - int32_t(col[1] + 2u * col[0]);
+  const int32_t Mt = int32_t(2u * rowsum[4] + rowsum[3]) - int32_t(rowsum[1] + 2u * rowsum[0]);
+  const uint32_t Mpp = 4u * (col[0] + col[4]) + col[1] + col[3];
+  const uint32_t Mtt = 4u * (rowsum[0] + rowsum[4]) + rowsum[1] + rowsum[3];
+  const int32_t tglob = t_row0 + int32_t(j);                            // t_row0 = global time of map row 0
   uint32_t flags = 0;
   if (pad < 2u || pad + 2u >= npads) flags |= 1u;                       // D8 EDGE_PAD
   if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
-  if (qP == kQClamp || (meta & 0xFF00u)) flags |= 4u;                   // SATURATED
-  if (meta >> 16) flags |= 8u;                                          // SPLIT
-  lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob),
-                  qP | (((meta & 0xFFu) + 1u) << 16), Wsum);
+  if (nsat) flags |= 4u;                                                // SATURATED
+  if (nsplit) flags |= 8u;                                              // SPLIT
+  lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob), qP | (ncells << 16), Wsum);
   hi = make_uint4(uint32_t(Mp), uint32_t(Mt), Mpp, Mtt);
 }
 
@@ -243,6 +252,10 @@ __device__ __forceinline__ void finish_rec(uint4& lo, uint4& hi) {
 //            <=> Q >= max(early + 1, late, theta)
 // The compare is a half2 compare on the raw bit patterns: all operands are <= 16369 < 0x7C00, i.e.
 // non-negative finite fp16 values (denormals included) whose order is the integer order.
+// The words left and right of a strip come from the neighbour lanes' registers (consecutive lanes hold
+// consecutive strips of a row; lanes 0 and 31 load them).  At a row's left end the word is zero by
+// construction: the map's last two columns are never written, and the neighbour lane's (or the loaded) word
+// there is the last word of a row.  At the right end it is forced to zero.
 // ----------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t shifted_pair(uint32_t w_left, uint32_t w) { return __byte_perm(w_left, w, 0x5432); }
 __device__ __forceinline__ uint32_t ge_mask2(uint32_t a, uint32_t b) {   // 0xFFFF per half where a >= b
@@ -257,16 +270,16 @@ struct SweepRow {          // what the sweep keeps of one time row, per strip of
   uint32_t E1[4];          // max(H3 of the row above, S_i) + 1: the early side, ready for the compare
 };
 
-// Load row j of strip s, derive S / H3 / E1 (`cur`), and emit the flag byte of row j-1 (`prev`).
-__device__ __forceinline__ uint32_t sweep_step(const uint16_t* __restrict__ map, uint32_t W, uint32_t j, uint32_t s,
-                                               uint32_t ns, uint32_t lane, uint32_t theta2, const SweepRow& prev,
-                                               SweepRow& cur) {
-  const uint32_t cell0 = j * W + 8u * s;
-  const uint4 c = *reinterpret_cast<const uint4*>(map + cell0);
+// Load the strip at shared address a (row j), derive S / H3 (/ E1) into `cur`, and (kTest) return the flag byte
+// of row j-1 (`prev`).
+template <bool kE1, bool kTest>
+__device__ __forceinline__ uint32_t sweep_step(uint32_t a, bool lane_first, bool lane_last, bool row_end, uint32_t theta2,
+                                               const SweepRow& prev, SweepRow& cur) {
+  const uint4 c = lds128(a);
   uint32_t wl = __shfl_up_sync(0xffffffffu, c.w, 1), wr = __shfl_down_sync(0xffffffffu, c.x, 1);
-  const uint32_t* m32 = reinterpret_cast<const uint32_t*>(map) + (cell0 >> 1);
-  if (s == 0u) wl = 0u; else if (lane == 0u) wl = m32[-1];              // (the map's columns 0,1 are zero anyway)
-  if (s + 1u == ns) wr = 0u; else if (lane == 31u) wr = m32[4];
+  if (lane_first) wl = lds32(a - 4u);
+  if (lane_last) wr = lds32(a + 16u);
+  if (row_end) wr = 0u;   // (the next lane may be the last segment reading past the map: not a row start)
   const uint32_t S0 = shifted_pair(wl, c.x), S1 = shifted_pair(c.x, c.y), S2 = shifted_pair(c.y, c.z),
                  S3 = shifted_pair(c.z, c.w), S4 = shifted_pair(c.w, wr);
   cur.C[0] = c.x; cur.C[1] = c.y; cur.C[2] = c.z; cur.C[3] = c.w;
@@ -275,23 +288,28 @@ __device__ __forceinline__ uint32_t sweep_step(const uint16_t* __restrict__ map,
   cur.H3[1] = __vimax3_u16x2(S1, c.y, S2);
   cur.H3[2] = __vimax3_u16x2(S2, c.z, S3);
   cur.H3[3] = __vimax3_u16x2(S3, c.w, S4);
-  cur.E1[0] = __vmaxu2(prev.H3[0], S0) + 0x00010001u;
-  cur.E1[1] = __vmaxu2(prev.H3[1], S1) + 0x00010001u;
-  cur.E1[2] = __vmaxu2(prev.H3[2], S2) + 0x00010001u;
-  cur.E1[3] = __vmaxu2(prev.H3[3], S3) + 0x00010001u;
-  // row j-1: late side needs H3 of this row
+  if (kE1) {
+    cur.E1[0] = __vmaxu2(prev.H3[0], S0) + 0x00010001u;
+    cur.E1[1] = __vmaxu2(prev.H3[1], S1) + 0x00010001u;
+    cur.E1[2] = __vmaxu2(prev.H3[2], S2) + 0x00010001u;
+    cur.E1[3] = __vmaxu2(prev.H3[3], S3) + 0x00010001u;
+  }
+  if constexpr (!kTest) {
+    return 0u;
+  } else {
+  // row j-1: the late side needs H3 of this row
   uint32_t M[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    const uint32_t late = __vmaxu2(cur.H3[i], prev.Sr[i]);
-    const uint32_t X = __vimax3_u16x2(prev.E1[i], late, theta2);
+    const uint32_t X = __vimax3_u16x2(__vmaxu2(cur.H3[i], prev.Sr[i]), prev.E1[i], theta2);
     M[i] = ge_mask2(prev.C[i], X);
   }
   // gather the eight flags into one byte, bit b <-> column 8 s + b: word i's low half at bit 2i, high half at 2i+1
-  const uint32_t a = bitsel(0x00020001u, M[0], M[1]);
-  const uint32_t b = bitsel(0x00200010u, M[2], M[3]);
-  const uint32_t sel = bitsel(0x000A0005u, a, b);
+  const uint32_t x = bitsel(0x00020001u, M[0], M[1]);
+  const uint32_t y = bitsel(0x00200010u, M[2], M[3]);
+  const uint32_t sel = bitsel(0x000A0005u, x, y);
   return bitsel(0x55u, sel, sel >> 16);                                 // low byte is the flag byte
+  }
 }
 
 // ----------------------------------------------------------------------------------------
@@ -300,8 +318,9 @@ __device__ __forceinline__ uint32_t sweep_step(const uint16_t* __restrict__ map,
 constexpr int kBarWork = 1, kBarFull = 2, kBarEmpty = 4;
 constexpr uint32_t kStopTile = 0xFFFFFFFFu;
 constexpr int kWorkWarps = kWorkThreads / 32;
-constexpr int kWarpList = 64;                 // peaks a warp lists per round (its 16 core rows)
-static_assert(kWorkWarps * 16 == kTileT, "every worker warp owns 16 core rows of a tile");
+constexpr int kMapGuard = 16;                 // zero bytes in front of and behind the map (the sweep's edge loads)
+static_assert(kWorkWarps * 16 == kTileT, "lanes 0..15 of every worker warp own one core row of a tile each");
+static_assert(kListCap <= kWorkThreads, "one thread per listed peak");
 __device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -310,18 +329,19 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
   uint8_t* sp = smem_raw;                                   // __align__(128); no static shared memory before it
-  uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // map, then flag bytes
+  uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // guard, map, guard, flag bytes
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
-  uint32_t* wlist = reinterpret_cast<uint32_t*>(sp);        sp += kWorkWarps * kWarpList * 4;
+  uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;  // 16-byte aligned entries
+  uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;      // peaks of the current item
   uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // next tile: index, sector, row, tile of the row
   uint32_t* wtot = reinterpret_cast<uint32_t*>(sp);         sp += 32 * 4;        // peaks per worker warp
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
-  uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;
-  uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 12 * 4;        // D6: L / S for S = 1..9
+  uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 16 * 4;        // D6: L / S for S = 1..9
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   for (uint32_t i = tid; i < uint32_t(kNbrTabWords); i += kThreads) nbr_tab[i] = nbr_tab_entry(i);
-  if (tid < 9u) wtab[tid] = kShareL / (tid + 1u);
+  if (tid < 16u) wtab[tid] = tid < 9u ? kShareL / (tid + 1u) : 0u;
+  for (uint32_t i = tid; i < uint32_t(kMapGuard) / 4u; i += kThreads) reinterpret_cast<uint32_t*>(mapraw)[i] = 0u;
   __syncthreads();
 
   if (warp == uint32_t(kWorkWarps)) {
@@ -355,9 +375,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   }
 
   // ================= worker warps =================
-  const uint32_t sub = lane & 3u;                                      // four lanes per peak: lane frame R_sub
-  const int32_t rot_cs = (sub == 0u) ? 1 : (sub == 2u) ? -1 : 0, rot_sn = (sub == 1u) ? 1 : (sub == 3u) ? -1 : 0;
-  const uint32_t theta2 = P.theta | (P.theta << 16);
+  const uint32_t theta2 = P.theta2;
+  const uint32_t map_s = smem_u32(mapraw) + uint32_t(kMapGuard);        // shared-space address of the map
+  const uint32_t tab_s = smem_u32(nbr_tab), wtab_s = smem_u32(wtab);
+  uint16_t* map = reinterpret_cast<uint16_t*>(mapraw + kMapGuard);
   // address and (clamped) length of a tile's digit list (tile = bin: kTileT == kBinT)
   auto tile_list = [&](uint32_t t, uint32_t sector, uint32_t row, uint32_t tt, const uint32_t*& src) -> uint32_t {
     const uint32_t cap = P.rows[row].cap;
@@ -384,20 +405,19 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     const RowInfo ri = P.rows[row];
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
-    const uint32_t W = ri.W, ns = W >> 3;
-    const uint32_t fpb = flag_pitch_bytes(W), nfw = fpb >> 2;
-    uint16_t* map = reinterpret_cast<uint16_t*>(mapraw);
-    uint8_t* fl = mapraw + uint32_t(kBoxH) * W * 2u;                     // W % 8 == 0: 16-byte aligned
-    const uint32_t* fw = reinterpret_cast<const uint32_t*>(fl);
+    const uint32_t W = ri.W, pitch = 2u * W, fpb = ri.fpb, nfw = fpb >> 2;
+    const uint32_t flag_off = uint32_t(kBoxH) * pitch + uint32_t(kMapGuard);   // flag bytes follow the map and its guard
+    const uint32_t flag_s = map_s + flag_off;
+    const uint32_t* fw = reinterpret_cast<const uint32_t*>(mapraw + kMapGuard + flag_off);
     const uint32_t* src;
     const uint32_t n = tile_list(t, sector, row, tt, src);              // k_bin: a multiple of 8; 0 entries are padding
     const uint4* src4 = reinterpret_cast<const uint4*>(src);
     const uint32_t n4 = n >> 2;
 
-    // ---- D2: zero the tile's charge map and flag bytes ----
+    // ---- D2: zero the tile's charge map, the guard behind it and the flag bytes ----
     {
-      const uint32_t nz = (uint32_t(kBoxH) * W * 2u + uint32_t(kBoxH) * fpb + 15u) >> 4;
-      uint4* z = reinterpret_cast<uint4*>(mapraw);
+      const uint32_t nz = (flag_off + uint32_t(kBoxH) * fpb + 15u) >> 4;
+      uint4* z = reinterpret_cast<uint4*>(mapraw + kMapGuard);
       for (uint32_t i = tid; i < nz; i += kWorkThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     bar_sync_named(kBarWork, kWorkThreads);
@@ -424,45 +444,41 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     bar_sync_named(kBarWork, kWorkThreads);
 
     // ---- S2: dense D4 sweep -> flag bytes of map rows 1 .. kBoxH-2 ----
-    {
-      // tasks = (strip s, row segment g): consecutive threads take consecutive strips of one segment, so that a
-      // lane's horizontal neighbours are its neighbour lanes' registers
-      constexpr uint32_t kRowsOut = uint32_t(kBoxH) - 2u;                // 264
-      const uint32_t nseg_max = max(uint32_t(kWorkThreads) / ns, 1u);
-      const uint32_t L = (kRowsOut + nseg_max - 1u) / nseg_max;          // rows per segment
-      const uint32_t nseg = (kRowsOut + L - 1u) / L;
-      const uint32_t ntasks = ns * nseg;
-      for (uint32_t task0 = warp * 32u; task0 < ntasks; task0 += uint32_t(kWorkThreads)) {   // (one pass unless ns > kWorkThreads)
-        const uint32_t task = task0 + lane;
-        const bool active = task < ntasks;
-        const uint32_t g = active ? task / ns : 0u, s = active ? task - g * ns : 0u;
-        const uint32_t jbase = g * L;                                    // first row loaded; rows jbase+1 .. jbase+L are flagged
-        const uint32_t jlast = min(jbase + L, kRowsOut);                 // last row flagged by this task
-        SweepRow ra, rb;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) { ra.C[i] = ra.Sr[i] = ra.H3[i] = ra.E1[i] = 0u; }
-        rb = ra;
-        // step k loads row jbase + k and flags row jbase + k - 1 (valid from k = 2 on)
-        for (uint32_t k = 0; k < L + 2u; k += 2u) {
-          {
-            const uint32_t j = min(jbase + k, uint32_t(kBoxH) - 1u);
-            const uint32_t byte = sweep_step(map, W, j, s, ns, lane, theta2, ra, rb);
-            const uint32_t jo = jbase + k - 1u;
-            if (active && k >= 2u && jo <= jlast) fl[jo * fpb + 4u + s] = uint8_t(byte);
-          }
-          {
-            const uint32_t j = min(jbase + k + 1u, uint32_t(kBoxH) - 1u);
-            const uint32_t byte = sweep_step(map, W, j, s, ns, lane, theta2, rb, ra);
-            const uint32_t jo = jbase + k;
-            if (active && k >= 1u && jo <= jlast) fl[jo * fpb + 4u + s] = uint8_t(byte);
-          }
-        }
+    // tasks = (strip s, row segment g): consecutive threads take consecutive strips of one segment, so that a
+    // lane's horizontal neighbours are its neighbour lanes' registers.  Segment g loads rows g L .. g L + L + 1
+    // and flags rows g L + 1 .. g L + L.
+    for (uint32_t task0 = warp * 32u; task0 < ri.ntasks; task0 += uint32_t(kWorkThreads)) {   // (one pass unless the row has > 512 strips x segments)
+      const uint32_t task = task0 + lane, L = ri.segL, ns = ri.ns;
+      const bool active = task < ri.ntasks;
+      const uint32_t g = active ? (task * ri.rcp_ns) >> 16 : 0u, s = active ? task - g * ns : 0u;
+      const uint32_t jbase = g * L;
+      const uint32_t nout = active ? min(L, uint32_t(kBoxH) - 2u - jbase) : 0u;   // rows flagged by this task
+      // (the last segment reads up to L + 1 rows past the map: flag bytes and staging, always inside this CTA's
+      //  shared memory; what it derives from them only feeds flag bytes that are not stored)
+      uint32_t a = map_s + jbase * pitch + 16u * s;
+      uint32_t f = flag_s + (jbase + 1u) * fpb + 4u + s;
+      const bool lf = lane == 0u, ll = lane == 31u, re = s + 1u == ns;
+      SweepRow ra, rb;
+      sweep_step<false, false>(a, lf, ll, re, theta2, ra, ra);
+      a += pitch;
+      sweep_step<true, false>(a, lf, ll, re, theta2, ra, rb);
+      a += pitch;
+      for (uint32_t m = 0; m < L; m += 2u) {
+        const uint32_t b0 = sweep_step<true, true>(a, lf, ll, re, theta2, rb, ra);
+        a += pitch;
+        if (m < nout) sts8(f, b0);
+        f += fpb;
+        if (m + 1u >= L) break;
+        const uint32_t b1 = sweep_step<true, true>(a, lf, ll, re, theta2, ra, rb);
+        a += pitch;
+        if (m + 1u < nout) sts8(f, b1);
+        f += fpb;
       }
     }
     bar_sync_named(kBarWork, kWorkThreads);   // flags complete
 
     // ---- S6 (in-tile part): ordered count; lanes 0..15 of warp w own the core rows 16 w .. 16 w + 15 ----
-    const uint32_t krow = warp * 16u + (lane & 15u);                     // core row of this lane (lanes 16..31 mirror 0..15)
+    const uint32_t krow = warp * 16u + (lane & 15u);
     const uint32_t jrow = uint32_t(kReach) + krow;
     uint32_t cnt = 0;
     if (lane < 16u && krow < ncore) {
@@ -494,46 +510,38 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
     // publish the tile's count early so that later tiles' look-backs never wait for this tile's build
     if (tid == 0 && t != 0u) st_release_u64(P.tile_state + t, pack_state(P.epoch, kStAgg, total));
 
-    // ---- S3..S5: every warp builds the clusters of its own rows; at most kListCap records per hand-over item ----
+    // ---- S3..S5: at most kListCap peaks per hand-over item: list them in order, then one thread per peak ----
     const uint32_t sector_row = sector | (row << 8);
     const int32_t t_row0 = t0 - kReach;
+    const uint32_t rowfirst = wbase + lexcl;                             // tile index of this lane's row's first peak
     uint32_t done = 0;
     do {
       const uint32_t b = q & 1u;
-      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
       const uint32_t npass = min(total - done, uint32_t(kListCap));
-      uint4* stg = stage + b * (2u * kListCap);
-      // this warp's peaks are the tile's peaks wbase .. wbase + wcount - 1; those inside [done, done + npass) go now
-      // (warp-local indices first .. last-1; empty when first >= last)
-      const uint32_t first = done > wbase ? min(done - wbase, wcount) : 0u;
-      const uint32_t last = done + npass > wbase ? min(done + npass - wbase, wcount) : 0u;
-      for (uint32_t r0 = first; r0 < last; r0 += uint32_t(kWarpList)) {
-        const uint32_t r1 = min(r0 + uint32_t(kWarpList), last);
-        // list the warp's peaks r0 .. r1-1: the row owners walk their flag bits in ascending pad order
-        uint32_t* wl = wlist + warp * uint32_t(kWarpList);
-        __syncwarp();
-        if (lane < 16u && cnt != 0u && lexcl < r1 && lexcl + cnt > r0) {
-          const uint32_t* r = fw + jrow * nfw;
-          uint32_t k = lexcl;
-          for (uint32_t w = 1; w < nfw; ++w) {
-            uint32_t bits = r[w];
-            while (bits) {
-              const uint32_t bpos = uint32_t(__ffs(bits)) - 1u;
-              bits &= bits - 1u;
-              if (k >= r0 && k < r1) wl[k - r0] = (jrow << 8) | ((w - 1u) * 32u + bpos - uint32_t(kColOff));
-              ++k;
-            }
+      // the row owners walk their flag bits in ascending pad order
+      if (lane < 16u && cnt != 0u && rowfirst < done + npass && rowfirst + cnt > done) {
+        const uint32_t* r = fw + jrow * nfw;
+        uint32_t k = rowfirst;
+        for (uint32_t w = 1; w < nfw; ++w) {
+          uint32_t bits = r[w];
+          while (bits) {
+            const uint32_t bpos = uint32_t(__ffs(bits)) - 1u;
+            bits &= bits - 1u;
+            if (k - done < npass) plist[k - done] = (jrow << 8) | ((w - 1u) * 32u + bpos - uint32_t(kColOff));
+            ++k;
           }
         }
-        __syncwarp();
-        for (uint32_t i0 = r0; i0 < r1; i0 += 8u) {
-          const uint32_t i = min(i0 + (lane >> 2), r1 - 1u);             // (a ragged group redoes the last peak)
-          const uint32_t e = wl[i - r0];
-          uint4 lo4, hi4;
-          build4(map, fw, W, nfw, e >> 8, e & 0xFFu, nbr_tab, wtab, sub, rot_cs, rot_sn, sector_row, ri.npads, t_row0,
-                 P.tf_time_bins, lo4, hi4);
-          if (i0 + (lane >> 2) < r1 && sub < 2u) stg[2u * (wbase + i - done) + sub] = sub ? hi4 : lo4;
-        }
+      }
+      bar_sync_named(kBarWork, kWorkThreads);                           // the list is complete
+      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
+      if (tid < npass) {
+        const uint32_t e = plist[tid];
+        uint4 lo4, hi4;
+        build1(map_s, flag_s, pitch, fpb, e >> 8, e & 0xFFu, tab_s, wtab_s, sector_row, ri.npads, t_row0, P.tf_time_bins,
+               lo4, hi4);
+        uint4* stg = stage + b * (2u * kListCap) + 2u * tid;
+        stg[0] = lo4;
+        stg[1] = hi4;
       }
       if (tid == 0) {
         uint32_t* m = s_meta + 4u * b;
@@ -545,6 +553,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       bar_arrive_named(kBarFull + int(b), kThreads);                     // the records of this item are staged
       ++q;
       done += npass;
+      if (done < total) bar_sync_named(kBarWork, kWorkThreads);         // the list is reused
     } while (done < total);
     bar_sync_named(kBarWork, kWorkThreads);   // map, flags and s_next are stable until here
   }
