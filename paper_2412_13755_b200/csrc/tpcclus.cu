@@ -187,10 +187,10 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     ri.ns = uint16_t(ri.W / 8);
     ri.fpb = uint16_t(flag_pitch_bytes(ri.W));
     {
-      // sweep tasks: as many row segments as the worker threads can take at once, each flagging segL of the
-      // kBoxH - 2 rows that carry flags
+      // sweep tasks: as many row segments as the worker warps can take at once (30 tasks per warp: two lanes
+      // repeat the neighbouring tasks), each flagging segL of the kBoxH - 2 rows that carry flags
       const uint32_t rows_out = uint32_t(kBoxH) - 2u;
-      const uint32_t nseg_max = std::max<uint32_t>(uint32_t(kWorkThreads) / ri.ns, 1u);
+      const uint32_t nseg_max = std::max<uint32_t>(uint32_t(kWorkWarps) * 30u / ri.ns, 1u);
       const uint32_t L = (rows_out + nseg_max - 1) / nseg_max;
       ri.segL = uint16_t(L);
       ri.ntasks = uint16_t(ri.ns * ((rows_out + L - 1) / L));
@@ -210,8 +210,8 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kNbrTabWords * 4 + kListCap * 4 + 16 + 32 * 4 + 2 * 4 * 4 +
-                  16 * 4 + 128;
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kNbrTabWords * 4 + kTileT * 4 + kWorkWarps * kWorkWarps * 4 + 64 +
+                  32 * 4 + 2 * 4 * 4 + 16 * 4 + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;

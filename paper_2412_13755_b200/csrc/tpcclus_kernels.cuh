@@ -27,17 +27,21 @@
 
 namespace tpcclus {
 
-constexpr int      kThreads      = 544;   // CTA size of k_tile (two CTAs per SM): 16 worker warps + the committer warp
-constexpr int      kWorkThreads  = 512;   // warps 0..15 work on the tile; warp 16 commits
-constexpr int      kTileT        = 256;   // core time bins per tile (= one digit bin of k_bin)
+#ifndef TPCCLUS_TILE_T
+#define TPCCLUS_TILE_T 256
+#endif
+constexpr int      kTileT        = TPCCLUS_TILE_T;   // core time bins per tile (= one digit bin of k_bin)
+constexpr int      kWorkThreads  = 2 * kTileT;       // worker warps of k_tile: one per 16 core rows
+constexpr int      kThreads      = kWorkThreads + 32;   // + the committer warp
+constexpr int      kTileCtasPerSm = kTileT == 256 ? 2 : 4;
 constexpr int      kReach        = 5;     // D9: charges within Chebyshev distance 5 decide a cluster
 constexpr int      kBoxH         = kTileT + 2 * kReach;   // map rows of a tile (266)
-constexpr int      kBinT         = 256;   // core time bins per digit bin
-constexpr int      kBinShift     = 8;
+constexpr int      kBinT         = kTileT;   // core time bins per digit bin
+constexpr int      kBinShift     = kTileT == 256 ? 8 : 7;
 constexpr int      kBinBoxH      = kBinT + 2 * kReach;    // time rows a bin's window spans (266)
 static_assert((1 << kBinShift) == kBinT && kBinT == kTileT, "a digit bin is one tile");
 constexpr int      kColOff       = 2;     // map column of pad 0 (two zero columns each side: 5x5 window)
-constexpr int      kListCap      = 256;   // records per hand-over item (capacity of one staging buffer)
+constexpr int      kListCap      = kWorkThreads < 256 ? kWorkThreads : 256;   // records per hand-over item (capacity of one staging buffer)
 constexpr uint32_t kQClamp       = 16368; // D1
 constexpr int      kMaxSectors   = 256;
 

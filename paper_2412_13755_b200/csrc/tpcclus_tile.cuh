@@ -15,14 +15,17 @@
 //             byte store, so the flag map needs neither atomics nor clearing                   (S2)
 //   count     one lane per core row: popc of its flag words, warp scan, CTA scan -> the position of every
 //             peak in (time,pad) order; the tile's count is published for the look-back       (S6, S7)
-//   list      the row owners write their peaks, in order, into the tile's peak list
-//   build     one thread per peak, dense over the list: the 25 charges and the 9x9 flag window straight from
-//             the map (S3..S5); exact integer records (RawRec) go to a staging buffer
+//   build     one thread per peak, dense over the tile's peaks in order (each thread finds its peak by two short
+//             binary searches over the count prefixes and a bit select): the 25 charges and the 9x9 flag window
+//             straight from the map (S3..S5); exact integer records (RawRec) go to a staging buffer
 //   commit    the committer warp: decoupled look-back across tiles, D8 finish in fp64, ordered copy-out (S6)
 //
 // Definitions D1..D12: SURVEY.md §8(c), restated in DESIGN.md §2.  No code here is shared with oracle/.
 #pragma once
 #include <cuda_fp16.h>
+#ifdef TPCCLUS_PHASE_CLOCKS
+#include <cstdio>
+#endif
 
 namespace tpcclus {
 
@@ -135,20 +138,21 @@ __device__ __forceinline__ uint32_t nbr_tab_entry(uint32_t idx) {
 // window that starts four pads to the left of a peak addressable without a branch for p < 4.
 __host__ __device__ inline uint32_t flag_pitch_bytes(uint32_t W) { return 4u + (((W >> 3) + 3u) & ~3u); }
 
-// Build the cluster of the peak at map row j, pad `pad` (one thread).  map_s / flag_s / tab_s / wtab_s are
-// shared-space addresses of the tile's map, its flag bytes, the neighbour table and the L/S table.
-__device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t pitch /* 2 W */, uint32_t fpb, uint32_t j,
-                                       uint32_t pad, uint32_t tab_s, uint32_t wtab_s, uint32_t sector_row, uint32_t npads,
-                                       int32_t t_row0, uint32_t tf_time_bins, uint4& lo, uint4& hi) {
+// Build the cluster of the peak at map row j, pad `pad` (one thread) from the tile's map (pitch W cells), its
+// flag words (nfw per row), the neighbour table and the L/S table, all in shared memory.
+__device__ __forceinline__ void build1(const uint16_t* __restrict__ map, const uint32_t* __restrict__ fw, uint32_t W, uint32_t nfw,
+                                       uint32_t j, uint32_t pad, const uint4* __restrict__ tab, const uint32_t* __restrict__ wtab,
+                                       uint32_t sector_row, uint32_t npads, int32_t t_row0, uint32_t tf_time_bins, uint4& lo,
+                                       uint4& hi) {
   // ---- the 25 charges ----
   uint32_t q[25];
   {
-    const uint32_t base = map_s + j * pitch + 2u * (pad + uint32_t(kColOff));
+    const uint16_t* c = map + j * W + (pad + uint32_t(kColOff));
 #pragma unroll
     for (int dt = -2; dt <= 2; ++dt) {
-      const uint32_t rb = base + uint32_t(dt) * pitch;
+      const uint16_t* rb = c + dt * int32_t(W);
 #pragma unroll
-      for (int dp = -2; dp <= 2; ++dp) q[(dt + 2) * 5 + dp + 2] = lds16(rb + uint32_t(2 * dp));
+      for (int dp = -2; dp <= 2; ++dp) q[(dt + 2) * 5 + dp + 2] = rb[dp];
     }
   }
   // ---- the 9x9 flag window: R[k] = flags of row j-4+k, bit i <-> pad p-4+i ----
@@ -156,9 +160,9 @@ __device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t
   {
     const uint32_t b0 = pad + (32u + uint32_t(kColOff) - 4u);           // bit index of pad p-4 inside a flag row
     const uint32_t sh = b0 & 31u;
-    const uint32_t a0 = flag_s + (j - 4u) * fpb + 4u * (b0 >> 5);
+    const uint32_t* a0 = fw + (j - 4u) * nfw + (b0 >> 5);
 #pragma unroll
-    for (int k = 0; k < 9; ++k) R[k] = __funnelshift_r(lds32(a0 + uint32_t(k) * fpb), lds32(a0 + uint32_t(k) * fpb + 4u), sh) & 0x1FFu;
+    for (int k = 0; k < 9; ++k) R[k] = __funnelshift_r(a0[uint32_t(k) * nfw], a0[uint32_t(k) * nfw + 1u], sh) & 0x1FFu;
     R[4] &= ~(1u << 4);                                                  // P itself
   }
   // ---- D6: other peaks of the window -> S(c) - 1 per cell (nibbles) ----
@@ -166,7 +170,7 @@ __device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t
   {
     uint32_t G0 = R[0] | (R[1] << 9) | (R[2] << 18), G1 = R[3] | (R[4] << 9) | (R[5] << 18), G2 = R[6] | (R[7] << 9) | (R[8] << 18);
     auto add = [&](uint32_t b) {
-      const uint4 e = lds128(tab_s + 16u * b);
+      const uint4 e = tab[b];
       acc0 += e.x; acc1 += e.y; acc2 += e.z; acc3 += e.w;
     };
     while (G0) { const uint32_t b = __ffs(G0) - 1; G0 &= G0 - 1; add(b); }
@@ -175,7 +179,7 @@ __device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t
   }
   const uint32_t qP = q[12];
   uint32_t col[5] = {0u, 0u, 0u, 0u, 0u}, rowsum[5] = {0u, 0u, 0u, 0u, 0u};
-  uint32_t ncells = 1u, nsat = (qP == kQClamp) ? 1u : 0u, nsplit = 0u;
+  uint32_t ncells = 1u, nsplit = 0u;
 #pragma unroll
   for (int k = 0; k < 25; ++k) {
     if (k == 12) continue;
@@ -198,12 +202,11 @@ __device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t
     // D6: w = Q * L / S
     const uint32_t accw = (k < 8) ? acc0 : (k < 16) ? acc1 : (k < 24) ? acc2 : acc3;
     const uint32_t nib = (accw >> (4 * (k & 7))) & 15u;                  // S - 1
-    const uint32_t w = m ? qc * lds32(wtab_s + 4u * nib) : 0u;
+    const uint32_t w = m ? qc * wtab[nib] : 0u;
     col[dp + 2] += w;
     rowsum[dt + 2] += w;
     if (m) {
       ncells += 1u;
-      nsat += (qc == kQClamp) ? 1u : 0u;
       nsplit += nib;
     }
   }
@@ -217,7 +220,7 @@ __device__ __forceinline__ void build1(uint32_t map_s, uint32_t flag_s, uint32_t
   uint32_t flags = 0;
   if (pad < 2u || pad + 2u >= npads) flags |= 1u;                       // D8 EDGE_PAD
   if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
-  if (nsat) flags |= 4u;                                                // SATURATED
+  if (qP == kQClamp) flags |= 4u;       // SATURATED: no member exceeds its peak (D4, D5), so a saturated member implies a saturated peak
   if (nsplit) flags |= 8u;                                              // SPLIT
   lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob), qP | (ncells << 16), Wsum);
   hi = make_uint4(uint32_t(Mp), uint32_t(Mt), Mpp, Mtt);
@@ -252,10 +255,10 @@ __device__ __forceinline__ void finish_rec(uint4& lo, uint4& hi) {
 //            <=> Q >= max(early + 1, late, theta)
 // The compare is a half2 compare on the raw bit patterns: all operands are <= 16369 < 0x7C00, i.e.
 // non-negative finite fp16 values (denormals included) whose order is the integer order.
-// The words left and right of a strip come from the neighbour lanes' registers (consecutive lanes hold
-// consecutive strips of a row; lanes 0 and 31 load them).  At a row's left end the word is zero by
-// construction: the map's last two columns are never written, and the neighbour lane's (or the loaded) word
-// there is the last word of a row.  At the right end it is forced to zero.
+// The words left and right of a strip come from the neighbour lanes' registers: consecutive lanes hold
+// consecutive strips (tasks), lanes 0 and 31 of a warp repeat the task before / after the warp's 30 and store
+// nothing.  At a row's ends the neighbour word is zero by construction: the map's first two and last two
+// columns are never written, and the neighbour lane holds the last (first) word of some row there.
 // ----------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t shifted_pair(uint32_t w_left, uint32_t w) { return __byte_perm(w_left, w, 0x5432); }
 __device__ __forceinline__ uint32_t ge_mask2(uint32_t a, uint32_t b) {   // 0xFFFF per half where a >= b
@@ -273,13 +276,9 @@ struct SweepRow {          // what the sweep keeps of one time row, per strip of
 // Load the strip at shared address a (row j), derive S / H3 (/ E1) into `cur`, and (kTest) return the flag byte
 // of row j-1 (`prev`).
 template <bool kE1, bool kTest>
-__device__ __forceinline__ uint32_t sweep_step(uint32_t a, bool lane_first, bool lane_last, bool row_end, uint32_t theta2,
-                                               const SweepRow& prev, SweepRow& cur) {
+__device__ __forceinline__ uint32_t sweep_step(uint32_t a, uint32_t theta2, const SweepRow& prev, SweepRow& cur) {
   const uint4 c = lds128(a);
-  uint32_t wl = __shfl_up_sync(0xffffffffu, c.w, 1), wr = __shfl_down_sync(0xffffffffu, c.x, 1);
-  if (lane_first) wl = lds32(a - 4u);
-  if (lane_last) wr = lds32(a + 16u);
-  if (row_end) wr = 0u;   // (the next lane may be the last segment reading past the map: not a row start)
+  const uint32_t wl = __shfl_up_sync(0xffffffffu, c.w, 1), wr = __shfl_down_sync(0xffffffffu, c.x, 1);
   const uint32_t S0 = shifted_pair(wl, c.x), S1 = shifted_pair(c.x, c.y), S2 = shifted_pair(c.y, c.z),
                  S3 = shifted_pair(c.z, c.w), S4 = shifted_pair(c.w, wr);
   cur.C[0] = c.x; cur.C[1] = c.y; cur.C[2] = c.z; cur.C[3] = c.w;
@@ -320,20 +319,31 @@ constexpr uint32_t kStopTile = 0xFFFFFFFFu;
 constexpr int kWorkWarps = kWorkThreads / 32;
 constexpr int kMapGuard = 16;                 // zero bytes in front of and behind the map (the sweep's edge loads)
 static_assert(kWorkWarps * 16 == kTileT, "lanes 0..15 of every worker warp own one core row of a tile each");
-static_assert(kListCap <= kWorkThreads, "one thread per listed peak");
+static_assert(kListCap <= kWorkThreads, "one thread per peak of an item");
 __device__ __forceinline__ void bar_arrive_named(int id, int nthreads) {
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-__global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ TileParams P) {
+#ifdef TPCCLUS_PHASE_CLOCKS   // debugging aid: per-phase cycle totals of a few CTAs (printf at kernel end)
+#define PH_DECL long long ph_t = clock64(); long long ph_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#define PH_MARK(i) { const long long ph_n = clock64(); ph_acc[i] += ph_n - ph_t; ph_t = ph_n; }
+#define PH_DUMP(ntiles) if (threadIdx.x == 0 && (blockIdx.x % 97) == 0) printf("cta %d tiles %u cycles: zero %lld scatter %lld sweep %lld count %lld build %lld endbar %lld top %lld waitempty %lld\n", int(blockIdx.x), ntiles, ph_acc[0], ph_acc[1], ph_acc[2], ph_acc[3], ph_acc[7], ph_acc[5], ph_acc[6], ph_acc[4]);
+#else
+#define PH_DECL
+#define PH_MARK(i)
+#define PH_DUMP(n)
+#endif
+
+__global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_constant__ TileParams P) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   // carve-up
   uint8_t* sp = smem_raw;                                   // __align__(128); no static shared memory before it
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // guard, map, guard, flag bytes
   uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
   uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;  // 16-byte aligned entries
-  uint32_t* plist = reinterpret_cast<uint32_t*>(sp);        sp += kListCap * 4;      // peaks of the current item
-  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 16;            // next tile: index, sector, row, tile of the row
+  uint32_t* rowx = reinterpret_cast<uint32_t*>(sp);         sp += kTileT * 4;        // per core row: peaks of its warp's earlier rows
+  uint32_t* wpre = reinterpret_cast<uint32_t*>(sp);         sp += kWorkWarps * kWorkWarps * 4;   // per warp: a copy of the warps' exclusive peak prefix
+  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 64;            // next tile (kNx* words) + its RowInfo (8 words)
   uint32_t* wtot = reinterpret_cast<uint32_t*>(sp);         sp += 32 * 4;        // peaks per worker warp
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
   uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 16 * 4;        // D6: L / S for S = 1..9
@@ -377,40 +387,51 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
   // ================= worker warps =================
   const uint32_t theta2 = P.theta2;
   const uint32_t map_s = smem_u32(mapraw) + uint32_t(kMapGuard);        // shared-space address of the map
-  const uint32_t tab_s = smem_u32(nbr_tab), wtab_s = smem_u32(wtab);
   uint16_t* map = reinterpret_cast<uint16_t*>(mapraw + kMapGuard);
-  // address and (clamped) length of a tile's digit list (tile = bin: kTileT == kBinT)
-  auto tile_list = [&](uint32_t t, uint32_t sector, uint32_t row, uint32_t tt, const uint32_t*& src) -> uint32_t {
-    const uint32_t cap = P.rows[row].cap;
-    src = P.lists + uint64_t(sector) * P.sec_list_elems + P.rows[row].list_off + uint64_t(tt) * cap;
-    return min(P.counts[t], cap);
-  };
-  // take the next tile in ticket order (one thread)
+  // take the next tile in ticket order (one thread) and leave everything the CTA needs to start on it in shared
+  // memory: indices, the row's constants, address and (clamped) length of its digit list (tile = bin)
   auto fetch = [&]() {
     const uint32_t t = atomicAdd(&P.status->ticket, 1u);
-    const uint32_t sr = t / P.tiles_per_row, sector = sr / P.n_rows;
     s_next[0] = t;
-    s_next[1] = sector;
-    s_next[2] = sr - sector * P.n_rows;         // row
-    s_next[3] = t - sr * P.tiles_per_row;       // tile of the row
+    if (t >= P.n_tiles) return;
+    const uint32_t sr = t / P.tiles_per_row, sector = sr / P.n_rows, row = sr - sector * P.n_rows, tt = t - sr * P.tiles_per_row;
+    const uint4* rp = reinterpret_cast<const uint4*>(P.rows + row);
+    const uint4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
+    const uint32_t cap = r0.y;
+    const uint64_t src = reinterpret_cast<uint64_t>(P.lists + uint64_t(sector) * P.sec_list_elems + r0.x + uint64_t(tt) * cap);
+    s_next[1] = sector | (row << 8);
+    s_next[2] = tt;
+    s_next[3] = min(__ldg(P.counts + t), cap);
+    s_next[4] = uint32_t(src);
+    s_next[5] = uint32_t(src >> 32);
+    *reinterpret_cast<uint4*>(s_next + 8) = r0;
+    *reinterpret_cast<uint4*>(s_next + 12) = r1;
   };
   if (tid == 0) fetch();
   bar_sync_named(kBarWork, kWorkThreads);
 
   uint32_t q = 0;                                                      // hand-over items issued so far
+  PH_DECL
+  uint32_t ph_tiles = 0;
   for (;;) {
     const uint32_t t = s_next[0];
     if (t >= P.n_tiles) break;
-    const uint32_t sector = s_next[1], row = s_next[2], tt = s_next[3];
-    const RowInfo ri = P.rows[row];
+    ++ph_tiles;
+    const uint32_t sector_row = s_next[1], tt = s_next[2], n = s_next[3];   // n: k_bin: a multiple of 8; 0 entries are padding
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(uint64_t(s_next[4]) | (uint64_t(s_next[5]) << 32));
+    RowInfo ri;
+    {
+      const uint4 r0 = *reinterpret_cast<const uint4*>(s_next + 8), r1 = *reinterpret_cast<const uint4*>(s_next + 12);
+      static_assert(sizeof(RowInfo) == 32, "two 16-byte words");
+      reinterpret_cast<uint4*>(&ri)[0] = r0;
+      reinterpret_cast<uint4*>(&ri)[1] = r1;
+    }
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
     const uint32_t W = ri.W, pitch = 2u * W, fpb = ri.fpb, nfw = fpb >> 2;
     const uint32_t flag_off = uint32_t(kBoxH) * pitch + uint32_t(kMapGuard);   // flag bytes follow the map and its guard
     const uint32_t flag_s = map_s + flag_off;
     const uint32_t* fw = reinterpret_cast<const uint32_t*>(mapraw + kMapGuard + flag_off);
-    const uint32_t* src;
-    const uint32_t n = tile_list(t, sector, row, tt, src);              // k_bin: a multiple of 8; 0 entries are padding
     const uint4* src4 = reinterpret_cast<const uint4*>(src);
     const uint32_t n4 = n >> 2;
 
@@ -420,7 +441,9 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       uint4* z = reinterpret_cast<uint4*>(mapraw + kMapGuard);
       for (uint32_t i = tid; i < nz; i += kWorkThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
+    PH_MARK(6)
     bar_sync_named(kBarWork, kWorkThreads);
+    PH_MARK(0)
     if (tid == 0) fetch();                    // next tile's ticket (s_next is read again after the tile's last barrier)
 
     // ---- S1: scatter the list into the map (16-byte loads, two in flight per thread) ----
@@ -442,40 +465,48 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       if (tid < (n & 3u)) put(__ldg(src + 4u * n4 + tid));               // k_bin_direct lists: any length
     }
     bar_sync_named(kBarWork, kWorkThreads);
+    PH_MARK(1)
 
     // ---- S2: dense D4 sweep -> flag bytes of map rows 1 .. kBoxH-2 ----
-    // tasks = (strip s, row segment g): consecutive threads take consecutive strips of one segment, so that a
-    // lane's horizontal neighbours are its neighbour lanes' registers.  Segment g loads rows g L .. g L + L + 1
-    // and flags rows g L + 1 .. g L + L.
-    for (uint32_t task0 = warp * 32u; task0 < ri.ntasks; task0 += uint32_t(kWorkThreads)) {   // (one pass unless the row has > 512 strips x segments)
-      const uint32_t task = task0 + lane, L = ri.segL, ns = ri.ns;
-      const bool active = task < ri.ntasks;
-      const uint32_t g = active ? (task * ri.rcp_ns) >> 16 : 0u, s = active ? task - g * ns : 0u;
-      const uint32_t jbase = g * L;
-      const uint32_t nout = active ? min(L, uint32_t(kBoxH) - 2u - jbase) : 0u;   // rows flagged by this task
-      // (the last segment reads up to L + 1 rows past the map: flag bytes and staging, always inside this CTA's
-      //  shared memory; what it derives from them only feeds flag bytes that are not stored)
-      uint32_t a = map_s + jbase * pitch + 16u * s;
-      uint32_t f = flag_s + (jbase + 1u) * fpb + 4u + s;
-      const bool lf = lane == 0u, ll = lane == 31u, re = s + 1u == ns;
+    // tasks = (strip s, row segment g): consecutive lanes take consecutive strips of one segment.  Segment g loads
+    // rows jb .. jb + L + 1 and flags rows jb + 1 .. jb + L, jb = min(g L, kBoxH - 2 - L) (the last segment is moved
+    // up so that nothing is read past the map; the rows it shares with its neighbour get the same bytes twice).
+    for (uint32_t task0 = warp * 30u; task0 < ri.ntasks; task0 += uint32_t(kWorkWarps) * 30u) {   // (one pass for the usual rows)
+      const uint32_t L = ri.segL, ns = ri.ns;
+      const int32_t tsk = int32_t(task0 + lane) - 1;
+      const bool owner = lane - 1u < 30u && uint32_t(tsk) < ri.ntasks;   // lanes 1..30 with a task of their own
+      const uint32_t task = tsk < 0 ? ri.ntasks - 1u : (uint32_t(tsk) < ri.ntasks ? uint32_t(tsk) : 0u);
+      const uint32_t g = (task * ri.rcp_ns) >> 16, s = task - g * ns;
+      const uint32_t jb = min(g * L, uint32_t(kBoxH) - 2u - L);
+      const uint32_t nout = owner ? L : 0u;
+      uint32_t a = map_s + jb * pitch + 16u * s;
+      uint32_t f = flag_s + (jb + 1u) * fpb + 4u + s;
       SweepRow ra, rb;
-      sweep_step<false, false>(a, lf, ll, re, theta2, ra, ra);
+      sweep_step<false, false>(a, theta2, ra, ra);
       a += pitch;
-      sweep_step<true, false>(a, lf, ll, re, theta2, ra, rb);
+      sweep_step<true, false>(a, theta2, ra, rb);
       a += pitch;
       for (uint32_t m = 0; m < L; m += 2u) {
-        const uint32_t b0 = sweep_step<true, true>(a, lf, ll, re, theta2, rb, ra);
+        const uint32_t b0 = sweep_step<true, true>(a, theta2, rb, ra);
         a += pitch;
         if (m < nout) sts8(f, b0);
         f += fpb;
         if (m + 1u >= L) break;
-        const uint32_t b1 = sweep_step<true, true>(a, lf, ll, re, theta2, ra, rb);
+        const uint32_t b1 = sweep_step<true, true>(a, theta2, ra, rb);
         a += pitch;
         if (m + 1u < nout) sts8(f, b1);
         f += fpb;
       }
     }
     bar_sync_named(kBarWork, kWorkThreads);   // flags complete
+    PH_MARK(2)
+    // pull the next tile's list towards L2 while this tile is counted and built (thread 0 fetched it after the
+    // first barrier of this tile)
+    if (s_next[0] < P.n_tiles) {
+      const uint32_t nn = s_next[3];
+      const uint32_t* nsrc = reinterpret_cast<const uint32_t*>(uint64_t(s_next[4]) | (uint64_t(s_next[5]) << 32));
+      for (uint32_t i = tid * 32u; i < nn; i += kWorkThreads * 32u) asm volatile("prefetch.global.L2 [%0];" ::"l"(nsrc + i));
+    }
 
     // ---- S6 (in-tile part): ordered count; lanes 0..15 of warp w own the core rows 16 w .. 16 w + 15 ----
     const uint32_t krow = warp * 16u + (lane & 15u);
@@ -491,55 +522,69 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
       if (lane >= uint32_t(o)) incl += v;
     }
-    const uint32_t lexcl = incl - cnt;                                   // peaks of this warp before this lane's row
     const uint32_t wcount = __shfl_sync(0xffffffffu, incl, 15);
+    if (lane < 16u) rowx[krow] = incl - cnt;                             // peaks of this warp before this lane's row
     if (lane == 0) wtot[warp] = wcount;
     bar_sync_named(kBarWork, kWorkThreads);
-    uint32_t wbase, total;
+    PH_MARK(3)
+    uint32_t total;
     {
       const uint32_t v = lane < uint32_t(kWorkWarps) ? wtot[lane] : 0u;
       uint32_t ps = v;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
+      for (int o = 1; o < kWorkWarps; o <<= 1) {
         const uint32_t u = __shfl_up_sync(0xffffffffu, ps, o);
         if (lane >= uint32_t(o)) ps += u;
       }
-      wbase = __shfl_sync(0xffffffffu, ps - v, warp);
+      if (lane < uint32_t(kWorkWarps)) wpre[warp * uint32_t(kWorkWarps) + lane] = ps - v;   // this warp's own copy
       total = __shfl_sync(0xffffffffu, ps, kWorkWarps - 1);
+      __syncwarp();
     }
     // publish the tile's count early so that later tiles' look-backs never wait for this tile's build
     if (tid == 0 && t != 0u) st_release_u64(P.tile_state + t, pack_state(P.epoch, kStAgg, total));
 
-    // ---- S3..S5: at most kListCap peaks per hand-over item: list them in order, then one thread per peak ----
-    const uint32_t sector_row = sector | (row << 8);
+    // ---- S3..S5: one thread per peak, at most kListCap peaks per hand-over item ----
     const int32_t t_row0 = t0 - kReach;
-    const uint32_t rowfirst = wbase + lexcl;                             // tile index of this lane's row's first peak
     uint32_t done = 0;
     do {
       const uint32_t b = q & 1u;
       const uint32_t npass = min(total - done, uint32_t(kListCap));
-      // the row owners walk their flag bits in ascending pad order
-      if (lane < 16u && cnt != 0u && rowfirst < done + npass && rowfirst + cnt > done) {
-        const uint32_t* r = fw + jrow * nfw;
-        uint32_t k = rowfirst;
+      PH_MARK(4)
+      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
+      PH_MARK(7)
+      const uint32_t pk = tid;                                          // one thread per peak, dense
+      if (pk < npass) {
+        // locate peak number done + pk of the tile in (time,pad) order: its warp (largest w with wpre[w] <= x),
+        // its row inside the warp's 16 (largest r with rowx[r] <= x'), then the x''-th set flag of that row
+        uint32_t x = done + pk;
+        const uint32_t* wp = wpre + warp * uint32_t(kWorkWarps);
+        uint32_t wsel = 0;
+#pragma unroll
+        for (int st = kWorkWarps / 2; st >= 1; st >>= 1)
+          if (wp[wsel + uint32_t(st)] <= x) wsel += uint32_t(st);
+        x -= wp[wsel];
+        const uint32_t* rx = rowx + wsel * 16u;
+        uint32_t rsel = 0;
+#pragma unroll
+        for (int st = 8; st >= 1; st >>= 1)
+          if (rx[rsel + uint32_t(st)] <= x) rsel += uint32_t(st);
+        x -= rx[rsel];
+        const uint32_t j = uint32_t(kReach) + wsel * 16u + rsel;
+        const uint32_t* r = fw + j * nfw;
+        uint32_t bits = 0, wbit = 0;
+        bool found = false;
         for (uint32_t w = 1; w < nfw; ++w) {
-          uint32_t bits = r[w];
-          while (bits) {
-            const uint32_t bpos = uint32_t(__ffs(bits)) - 1u;
-            bits &= bits - 1u;
-            if (k - done < npass) plist[k - done] = (jrow << 8) | ((w - 1u) * 32u + bpos - uint32_t(kColOff));
-            ++k;
+          const uint32_t v = r[w], c = __popc(v);
+          if (!found) {
+            if (x < c) { bits = v; wbit = (w - 1u) * 32u; found = true; } else x -= c;
           }
         }
-      }
-      bar_sync_named(kBarWork, kWorkThreads);                           // the list is complete
-      if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
-      if (tid < npass) {
-        const uint32_t e = plist[tid];
+        for (; x; --x) bits &= bits - 1u;                               // drop the x lowest flags
+        const uint32_t pad = wbit + uint32_t(__ffs(bits)) - 1u - uint32_t(kColOff);
         uint4 lo4, hi4;
-        build1(map_s, flag_s, pitch, fpb, e >> 8, e & 0xFFu, tab_s, wtab_s, sector_row, ri.npads, t_row0, P.tf_time_bins,
+        build1(map, fw, W, nfw, j, pad, reinterpret_cast<const uint4*>(nbr_tab), wtab, sector_row, ri.npads, t_row0, P.tf_time_bins,
                lo4, hi4);
-        uint4* stg = stage + b * (2u * kListCap) + 2u * tid;
+        uint4* stg = stage + b * (2u * kListCap) + 2u * pk;
         stg[0] = lo4;
         stg[1] = hi4;
       }
@@ -553,10 +598,13 @@ __global__ void __launch_bounds__(kThreads, 2) k_tile(const __grid_constant__ Ti
       bar_arrive_named(kBarFull + int(b), kThreads);                     // the records of this item are staged
       ++q;
       done += npass;
-      if (done < total) bar_sync_named(kBarWork, kWorkThreads);         // the list is reused
     } while (done < total);
+    PH_MARK(4)
     bar_sync_named(kBarWork, kWorkThreads);   // map, flags and s_next are stable until here
+    PH_MARK(5)
   }
+  PH_DUMP(ph_tiles)
+  (void)ph_tiles;
   // stop item
   {
     const uint32_t b = q & 1u;
