@@ -210,8 +210,8 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (tiles > 0x7FFFFFF0ull) return fail(TPCCLUS_ERR_GEOMETRY);
   c->max_tiles = uint32_t(tiles);
   c->max_bins = g->n_sectors * g->n_rows * c->bins_per_row_max;
-  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kNbrTabWords * 4 + kTileT * 4 + kWorkWarps * kWorkWarps * 4 + 64 +
-                  32 * 4 + 2 * 4 * 4 + 16 * 4 + 128;
+  c->smem_bytes = c->map_bytes_max + 2 * kListCap * 32 + kNbrTabWords * 4 + kTileT * 4 + kWorkWarps * kWorkWarps * 4 + 32 +
+                  32 * 4 + 2 * 4 * 4 + 16 * 4 + g->n_rows * uint32_t(sizeof(RowInfo)) + 128;
 
   int rc;
   const uint64_t list_bytes = uint64_t(g->n_sectors) * c->sec_list_elems * 4;

@@ -23,6 +23,9 @@
 // Definitions D1..D12: SURVEY.md §8(c), restated in DESIGN.md §2.  No code here is shared with oracle/.
 #pragma once
 #include <cuda_fp16.h>
+#ifndef TPCCLUS_BUILD_WARPS
+#define TPCCLUS_BUILD_WARPS 0   /* 0: dense (peak i -> thread i) */
+#endif
 #ifdef TPCCLUS_PHASE_CLOCKS
 #include <cstdio>
 #endif
@@ -343,14 +346,16 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
   uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;  // 16-byte aligned entries
   uint32_t* rowx = reinterpret_cast<uint32_t*>(sp);         sp += kTileT * 4;        // per core row: peaks of its warp's earlier rows
   uint32_t* wpre = reinterpret_cast<uint32_t*>(sp);         sp += kWorkWarps * kWorkWarps * 4;   // per warp: a copy of the warps' exclusive peak prefix
-  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 64;            // next tile (kNx* words) + its RowInfo (8 words)
+  uint32_t* s_next = reinterpret_cast<uint32_t*>(sp);       sp += 32;            // next tile: index, sector | row << 8, tile of the row, list length, list address
   uint32_t* wtot = reinterpret_cast<uint32_t*>(sp);         sp += 32 * 4;        // peaks per worker warp
   uint32_t* s_meta = reinterpret_cast<uint32_t*>(sp);       sp += 2 * 4 * 4;     // per staging buffer: tile, total, offset, count
   uint32_t* wtab = reinterpret_cast<uint32_t*>(sp);         sp += 16 * 4;        // D6: L / S for S = 1..9
+  uint4* s_rows = reinterpret_cast<uint4*>(sp);                                  // the RowInfo table, 2 x 16 bytes per row
 
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   for (uint32_t i = tid; i < uint32_t(kNbrTabWords); i += kThreads) nbr_tab[i] = nbr_tab_entry(i);
   if (tid < 16u) wtab[tid] = tid < 9u ? kShareL / (tid + 1u) : 0u;
+  for (uint32_t i = tid; i < 2u * P.n_rows; i += kThreads) s_rows[i] = __ldg(reinterpret_cast<const uint4*>(P.rows) + i);
   for (uint32_t i = tid; i < uint32_t(kMapGuard) / 4u; i += kThreads) reinterpret_cast<uint32_t*>(mapraw)[i] = 0u;
   __syncthreads();
 
@@ -388,26 +393,28 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
   const uint32_t theta2 = P.theta2;
   const uint32_t map_s = smem_u32(mapraw) + uint32_t(kMapGuard);        // shared-space address of the map
   uint16_t* map = reinterpret_cast<uint16_t*>(mapraw + kMapGuard);
-  // take the next tile in ticket order (one thread) and leave everything the CTA needs to start on it in shared
-  // memory: indices, the row's constants, address and (clamped) length of its digit list (tile = bin)
-  auto fetch = [&]() {
-    const uint32_t t = atomicAdd(&P.status->ticket, 1u);
+  // Tiles are taken by an atomic ticket in (sector,row,time) order, by thread 0, two tiles ahead: the ticket of
+  // tile t+2 and the list length of tile t+1 are requested at the start of tile t and only looked at phases later,
+  // so that neither round trip is ever waited for.  post() leaves what the CTA needs to start a tile in s_next.
+  auto post = [&](uint32_t t, uint32_t count) {
     s_next[0] = t;
     if (t >= P.n_tiles) return;
     const uint32_t sr = t / P.tiles_per_row, sector = sr / P.n_rows, row = sr - sector * P.n_rows, tt = t - sr * P.tiles_per_row;
-    const uint4* rp = reinterpret_cast<const uint4*>(P.rows + row);
-    const uint4 r0 = __ldg(rp), r1 = __ldg(rp + 1);
+    const uint4 r0 = s_rows[2u * row];                                   // list_off, cap, ...
     const uint32_t cap = r0.y;
     const uint64_t src = reinterpret_cast<uint64_t>(P.lists + uint64_t(sector) * P.sec_list_elems + r0.x + uint64_t(tt) * cap);
     s_next[1] = sector | (row << 8);
     s_next[2] = tt;
-    s_next[3] = min(__ldg(P.counts + t), cap);
+    s_next[3] = min(count, cap);                                          // k_bin: a multiple of 8; 0 entries are padding
     s_next[4] = uint32_t(src);
     s_next[5] = uint32_t(src >> 32);
-    *reinterpret_cast<uint4*>(s_next + 8) = r0;
-    *reinterpret_cast<uint4*>(s_next + 12) = r1;
   };
-  if (tid == 0) fetch();
+  uint32_t tk1 = 0, tk2 = 0, cnt1 = 0;                                   // thread 0: tickets of the next two tiles, next list length
+  if (tid == 0) {
+    const uint32_t tk0 = atomicAdd(&P.status->ticket, 1u);
+    tk1 = atomicAdd(&P.status->ticket, 1u);
+    post(tk0, tk0 < P.n_tiles ? __ldg(P.counts + tk0) : 0u);
+  }
   bar_sync_named(kBarWork, kWorkThreads);
 
   uint32_t q = 0;                                                      // hand-over items issued so far
@@ -417,14 +424,13 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     const uint32_t t = s_next[0];
     if (t >= P.n_tiles) break;
     ++ph_tiles;
-    const uint32_t sector_row = s_next[1], tt = s_next[2], n = s_next[3];   // n: k_bin: a multiple of 8; 0 entries are padding
+    const uint32_t sector_row = s_next[1], tt = s_next[2], n = s_next[3];
     const uint32_t* src = reinterpret_cast<const uint32_t*>(uint64_t(s_next[4]) | (uint64_t(s_next[5]) << 32));
     RowInfo ri;
     {
-      const uint4 r0 = *reinterpret_cast<const uint4*>(s_next + 8), r1 = *reinterpret_cast<const uint4*>(s_next + 12);
       static_assert(sizeof(RowInfo) == 32, "two 16-byte words");
-      reinterpret_cast<uint4*>(&ri)[0] = r0;
-      reinterpret_cast<uint4*>(&ri)[1] = r1;
+      reinterpret_cast<uint4*>(&ri)[0] = s_rows[2u * (sector_row >> 8)];
+      reinterpret_cast<uint4*>(&ri)[1] = s_rows[2u * (sector_row >> 8) + 1u];
     }
     const int32_t t0 = P.t_core_begin + int32_t(tt) * kTileT;           // global time of core row 0
     const uint32_t ncore = uint32_t(min(kTileT, P.t_core_end - t0));     // S7: only the core emits
@@ -444,7 +450,10 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     PH_MARK(6)
     bar_sync_named(kBarWork, kWorkThreads);
     PH_MARK(0)
-    if (tid == 0) fetch();                    // next tile's ticket (s_next is read again after the tile's last barrier)
+    if (tid == 0) {                           // requests for the tiles ahead (see above); nothing is waited for here
+      cnt1 = tk1 < P.n_tiles ? __ldg(P.counts + tk1) : 0u;
+      tk2 = atomicAdd(&P.status->ticket, 1u);
+    }
 
     // ---- S1: scatter the list into the map (16-byte loads, two in flight per thread) ----
     {
@@ -466,6 +475,10 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     }
     bar_sync_named(kBarWork, kWorkThreads);
     PH_MARK(1)
+    if (tid == 0) {                           // (every thread has read this tile's s_next before the first barrier)
+      post(tk1, cnt1);
+      tk1 = tk2;
+    }
 
     // ---- S2: dense D4 sweep -> flag bytes of map rows 1 .. kBoxH-2 ----
     // tasks = (strip s, row segment g): consecutive lanes take consecutive strips of one segment.  Segment g loads
@@ -500,8 +513,8 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     }
     bar_sync_named(kBarWork, kWorkThreads);   // flags complete
     PH_MARK(2)
-    // pull the next tile's list towards L2 while this tile is counted and built (thread 0 fetched it after the
-    // first barrier of this tile)
+    // pull the next tile's list towards L2 while this tile is counted and built (thread 0 posted it after the
+    // scatter barrier of this tile)
     if (s_next[0] < P.n_tiles) {
       const uint32_t nn = s_next[3];
       const uint32_t* nsrc = reinterpret_cast<const uint32_t*>(uint64_t(s_next[4]) | (uint64_t(s_next[5]) << 32));
@@ -552,7 +565,10 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
       PH_MARK(4)
       if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
       PH_MARK(7)
-      const uint32_t pk = tid;                                          // one thread per peak, dense
+      // one thread per peak; peak pk of the item goes to lane pk / kBuildWarps of warp pk % kBuildWarps, so that the
+      // long per-peak chains of several warps overlap
+      constexpr uint32_t kBuildWarps = TPCCLUS_BUILD_WARPS;
+      const uint32_t pk = kBuildWarps == 0u ? tid : (warp < kBuildWarps ? lane * kBuildWarps + warp : 0xFFFFFFFFu);
       if (pk < npass) {
         // locate peak number done + pk of the tile in (time,pad) order: its warp (largest w with wpre[w] <= x),
         // its row inside the warp's 16 (largest r with rowx[r] <= x'), then the x''-th set flag of that row
