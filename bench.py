@@ -83,21 +83,26 @@ def dist_max_sum(ms: float, units: float, world: int, device="cpu"):
 # clocks (profiling recipe: sample nvidia-smi DURING the timed region)
 # ----------------------------------------------------------------------------------------------
 class ClockSampler:
-    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown," \
+    """nvidia-smi sampled every 20 ms from BEFORE the warm-up (the process takes a few hundred ms to start); only
+    the samples whose timestamp falls inside the timed region [t0, t1] (host clock) are reported."""
+    Q = "timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown," \
         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown," \
         "clocks_event_reasons.sw_power_cap"
+    PERIOD_MS = 20
 
     def __init__(self, index=0):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", str(self.PERIOD_MS)],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
-    def stop(self):
-        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+    def stop(self, t0=None, t1=None):
+        import datetime
+
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0, period_ms=self.PERIOD_MS)
         if self.p is None:
             return out
         self.p.terminate()
@@ -111,13 +116,16 @@ class ClockSampler:
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             c = [x.strip() for x in line.split(",")]
-            if len(c) < 7:
+            if len(c) < 8:
                 continue
             try:
-                sm.append(float(c[0])); mx.append(float(c[1]))
+                ts = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                if t0 is not None and not (t0 <= ts <= t1):
+                    continue
+                sm.append(float(c[1])); mx.append(float(c[2]))
             except ValueError:
                 continue
-            for nme, v in zip(names, c[3:7]):
+            for nme, v in zip(names, c[4:8]):
                 if v.lower().startswith("active"):
                     reasons.add(nme)
         try:
@@ -128,6 +136,34 @@ class ClockSampler:
             out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
                        samples=len(sm))
         return out
+
+
+def kernel_source_sha256():
+    """Hash of the CUDA sources: profiles/traffic.json (ncu numbers) is stamped with it, and a bench line whose
+    kernels differ from the profiled ones says so instead of quoting stale counters."""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2412_13755_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_numbers(cfg_name):
+    """profiles/traffic.json: per-launch DRAM bytes and warp instructions per digit from the committed ncu capture,
+    keyed by workload; None when there is no entry for this workload."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    tj = json.load(open(p))
+    ent = tj.get("workloads", {}).get(cfg_name)
+    if ent is None:
+        return None
+    ent = dict(ent)
+    ent["stale"] = ent.get("source_sha256") != kernel_source_sha256()
+    return ent
 
 
 def measured_peak_gbs():
@@ -268,23 +304,28 @@ def run_ours(args):
             st = T.tpcclus_result(ctx)
             assert st["n_clusters"] == counts[i]
 
+    clocks = ClockSampler(local)              # started before the warm-up so that it is sampling by the timed region
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
     dist_barrier(world, local)
     T.tpcclus_set_profiling(ctx, True)
     launches0 = T.tpcclus_launch_count(ctx)
-    clocks = ClockSampler(local)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
+    wall0 = time.time()
     ev0.record()
     for _ in range(args.steps):
         step()
     ev1.record()
     torch.cuda.synchronize()
+    wall1 = time.time()
     dist_barrier(world, local)
     ms_total = ev0.elapsed_time(ev1)
-    clk = clocks.stop()
+    clk = clocks.stop(wall0, wall1)
+    if clk["samples"] < 5:
+        log(f"only {clk['samples']} clock samples inside the timed region ({ms_total:.1f} ms): raise --steps "
+            f"(>= {int(5 * ClockSampler.PERIOD_MS * 1.5 / max(ms_total / args.steps, 1e-3)) + 1} for this config)")
     launches = T.tpcclus_launch_count(ctx) - launches0
     prof, prof_runs = T.tpcclus_get_profile(ctx)
     T.tpcclus_set_profiling(ctx, False)
@@ -314,27 +355,32 @@ def run_ours(args):
                        achieved_gbs=alg[k] / (ms_avg * 1e-3) / 1e9 if ms_avg > 0 else None,
                        share=ms_sum / max(sum(prof.values()), 1e-9))
     dom = max(kern, key=lambda k: kern[k]["ms_per_launch"])
-    traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(dom) \
-        if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else None
+    # ncu counters of the committed capture of THIS workload (a C3 fragment is a C2 fragment: same generator, same
+    # size); null when the capture is of another workload, flagged when the kernels have changed since
+    fragment_like = {"C3-PbPb-TF": "C2-PbPb-fragment"}.get(cfg.name, cfg.name)
+    ncu = ncu_numbers(fragment_like)
+    traffic = ncu["dram_bytes_per_launch"].get(dom) if ncu else None
     # secondary, SM-side ceiling: both kernels are bound by instruction issue, not by HBM.
     # Warp instructions per launch come from the same ncu capture as `traffic` (they scale with the digits
     # of a launch); the peak is 4 schedulers x SMs x the SM clock sampled under load.
     issue = None
-    tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))) \
-        if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else {}
-    if "warp_inst_per_digit" in tj and clk.get("sm_mhz"):
+    if ncu and clk.get("sm_mhz"):
         import torch
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         peak_issue = 4.0 * n_sm * clk["sm_mhz"] * 1e6
         issue = {}
         for k in ("k_bin", "k_tile"):
-            wi = tj["warp_inst_per_digit"].get(k)
+            wi = ncu["warp_inst_per_digit"].get(k)
             if wi and kern[k]["ms_per_launch"] > 0:
                 ach = wi * n_dig / nfr / (kern[k]["ms_per_launch"] * 1e-3)
                 issue[k] = dict(warp_inst_per_launch=wi * n_dig / nfr, achieved=ach, peak=peak_issue,
                                 unit="warp-inst/s", frac=ach / peak_issue)
     roofline = dict(bound="hbm", kernel=dom, achieved=kern[dom]["achieved_gbs"], peak=peak, unit="GB/s",
                     frac=kern[dom]["achieved_gbs"] / peak, traffic=traffic, peak_source=peak_src,
+                    traffic_source=(dict(file="profiles/traffic.json", workload=fragment_like,
+                                         captured_on_source_sha256=ncu.get("source_sha256"),
+                                         this_source_sha256=kernel_source_sha256(), stale=ncu["stale"])
+                                    if ncu else None),
                     kernels=kern, issue=issue,
                     whole_step=dict(
                         b_min_bytes=8.0 * n_dig + 32.0 * n_cl,
@@ -343,26 +389,41 @@ def run_ours(args):
                         b_alg_bytes=sum(alg.values()) * nfr,
                         frac_b_alg=sum(alg.values()) * nfr / (ms_step_local * 1e-3) / 1e9 / peak))
 
-    # ---- cpu baseline (oracle, bounded sample) + parity spot check at full size ----
+    # ---- cpu baseline (oracle, bounded sample) + parity check at full size ----
+    # Sampled so that the first AND the last fragment and the first AND the last sectors are covered: the lower
+    # half of the sectors on fragment 0, the upper half (incl. sectors 32..35: the tail of k_bin's chunk ranges
+    # and k_tile's last tickets) on the last fragment (C3: the ragged 3776-bin one at the true TF end).
     cpu, parity = None, None
     if world == 1 and not args.no_cpu:
         cores = os.cpu_count() or 1
-        n_s = min(cfg.n_sectors, max(cores, 1) * 2)
-        f0 = tf[0]
-        a, b_ = 0, int(f0["offs"][n_s])
-        frag = dict(b=f0["b"], e=f0["e"], offs=f0["offs"],
-                    digits_np=gen.as_numpy_digits(f0["digits"][a:b_]))
-        dt, nd, res = oracle_sample(cfg, frag, list(range(n_s)), cores)
-        sample = f"{n_s} of {cfg.n_sectors} sectors of fragment 0 ({nd:,} digits), one sector per thread"
-        cpu = dict(value=nd / dt, unit=UNIT, cores=min(cores, n_s), kind="oracle", sample=sample, seconds=dt)
-        got = out[: counts[0]].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)
-        bad, nrec = 0, 0
-        for s, rec in res.items():
-            g = got[got["sector"] == s].copy()
-            g["sector"] = 0
-            nrec += len(rec)
-            bad += (len(g) != len(rec)) or (g.tobytes() != rec.tobytes())
-        parity = dict(fragment=0, sectors=n_s, records=nrec, sectors_not_bit_identical=int(bad))
+        ns = cfg.n_sectors
+        half = (ns + 1) // 2
+        plan = [(0, list(range(ns)))] if nfr == 1 else [(0, list(range(half))), (nfr - 1, list(range(half, ns)))]
+        bad, nrec, parts, t_cpu, nd_cpu = 0, 0, [], 0.0, 0
+        single = None
+        for fi, secs in plan:
+            fx = tf[fi]
+            a, b_ = int(fx["offs"][secs[0]]), int(fx["offs"][secs[-1] + 1])
+            offs_local = np.asarray(fx["offs"], dtype=np.int64) - a
+            frag = dict(b=fx["b"], e=fx["e"], offs=offs_local, digits_np=gen.as_numpy_digits(fx["digits"][a:b_]))
+            if single is None:      # the same oracle on ONE thread, one sector
+                dt1, nd1, _ = oracle_sample(cfg, frag, secs[:1], 1)
+                single = dict(value=nd1 / dt1, unit=UNIT, cores=1, seconds=dt1,
+                              sample=f"sector {secs[0]} of fragment {fi} ({nd1:,} digits)")
+            dt, nd, res = oracle_sample(cfg, frag, secs, cores)
+            t_cpu += dt
+            nd_cpu += nd
+            got = out[int(starts[fi]): int(starts[fi]) + counts[fi]].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)
+            for s_, rec in res.items():
+                g = got[got["sector"] == s_].copy()
+                g["sector"] = 0
+                nrec += len(rec)
+                bad += (len(g) != len(rec)) or (g.tobytes() != rec.tobytes())
+            parts.append(f"fragment {fi} sectors {secs[0]}..{secs[-1]}")
+        sample = f"{' + '.join(parts)} of {workload_name(cfg).split(':')[0]} ({nd_cpu:,} digits), one sector per thread"
+        cpu = dict(value=nd_cpu / t_cpu, unit=UNIT, cores=min(cores, half if nfr > 1 else ns), kind="oracle", sample=sample,
+                   seconds=t_cpu, single_thread=single)
+        parity = dict(checked=parts, records=nrec, sectors_not_bit_identical=int(bad))
 
     # ---- end to end through the C-ABI with HOST buffers (H2D + kernels + D2H inside the timing) ----
     e2e = None
@@ -439,6 +500,17 @@ def main():
     args = ap.parse_args()
     args.config = int(args.config) if args.config.isdigit() else args.config
     args.warmup = max(args.warmup, 0)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched bare: start the N replicas ourselves, one process per GPU, the way the driver would
+        # (torch.distributed.run, rendezvous on 127.0.0.1); rank 0 prints the JSON line
+        import socket
+
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

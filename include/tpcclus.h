@@ -37,13 +37,20 @@ extern "C" {
 #define TPCCLUS_OK             0
 #define TPCCLUS_ERR_INVALID   -1  /* null / misaligned pointer, core range larger than max_core_bins,
                                      core outside the TF, offsets not monotone, n > max_digits       */
-#define TPCCLUS_ERR_GEOMETRY  -2  /* npads out of 1..246, zero sizes, halo_bins in 1..4, tf > 65536   */
+#define TPCCLUS_ERR_GEOMETRY  -2  /* n_sectors / n_rows out of 1..256, npads out of 1..256, zero sizes,
+                                     halo_bins in 1..4 or > 4096, bin_occupancy_pct > 100,
+                                     tf_time_bins > TPCCLUS_MAX_TF_BINS, digit bins beyond 2^32 entries
+                                     per sector                                                       */
 #define TPCCLUS_ERR_CAPACITY  -3  /* more clusters than out_capacity: the first out_capacity records
                                      are valid and ordered, stats.n_clusters is the number required
                                      (hit count fluctuates -> "safety margin")         */
 #define TPCCLUS_ERR_DIGIT     -4  /* strict mode only: some digit was out of range / NaN / zero       */
 #define TPCCLUS_ERR_CUDA      -5  /* stats.cuda_error holds the cudaError_t                           */
 #define TPCCLUS_ERR_NOMEM     -6  /* device or pinned-host allocation failed in create                */
+#define TPCCLUS_ERR_OCCUPANCY -7  /* some (sector,row,256-bin) digit bin received more digits than
+                                     bin_occupancy_pct allows (scratch is sized ahead,
+                                     with a margin): the run's records are incomplete; create the
+                                     context with a larger bin_occupancy_pct                          */
 
 /* ---- cluster flag bits ---------------------------- */
 #define TPCCLUS_FLAG_EDGE_PAD   0x01u /* peak pad < 2 or >= npads[row]-2                      */
@@ -57,9 +64,15 @@ extern "C" {
 #define TPCCLUS_OPT_HOST_STAGING  0x0002u /* allocate the device staging buffers that
                                              tpcclus_run_host / tpcclus_run_tf_host need
                                              (2 x max_digits digits + 2 x max_clusters records) */
+#define TPCCLUS_OPT_BIN_DIRECT    0x0004u /* route digits with the plain one-atomic-per-entry binning
+                                             kernel (k_bin_direct) instead of the write-combining one;
+                                             same output bytes, slower.  It is what geometries with
+                                             more than 4096 digit bins per sector get anyway; the bit
+                                             exists so that tests can cover that kernel             */
 
 #define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
 #define TPCCLUS_MAX_NPADS  256u  /* the pad of a digit is a uint8 */
+#define TPCCLUS_MAX_TF_BINS 65536u /* the time of a digit is a uint16 */
 #define TPCCLUS_MAX_PENDING 64    /* runs that may be enqueued before their tpcclus_result */
 #define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
 
@@ -87,9 +100,9 @@ typedef struct {
 
 /* Detector shape and scratch sizing; read once by tpcclus_create (npads is copied). */
 typedef struct {
-  uint32_t n_sectors, n_rows;       /* 36, 152 in the configs; any >= 1                        */
+  uint32_t n_sectors, n_rows;       /* 36, 152 in the configs; each 1..256                     */
   const uint16_t* npads;            /* HOST array [n_rows], each 1..TPCCLUS_MAX_NPADS          */
-  uint32_t tf_time_bins;            /* whole-TF length, e.g. 57024; 1..65536 (u16 digit time)  */
+  uint32_t tf_time_bins;            /* whole-TF length, e.g. 57024; 1..TPCCLUS_MAX_TF_BINS    */
   uint32_t max_core_bins;           /* largest fragment core passed to run, e.g. 4096          */
   uint32_t halo_bins;               /* digits loaded each side of the core: 0 (single
                                        fragment) or >= TPCCLUS_MIN_HALO; 8 in configs[3]       */
@@ -98,6 +111,13 @@ typedef struct {
   uint16_t options;                 /* TPCCLUS_OPT_* bits                                      */
   uint64_t max_digits;              /* largest n passed to run                                 */
   uint64_t max_clusters;            /* sizing of the host-staging cluster buffers only         */
+  uint32_t bin_occupancy_pct;       /* capacity of a digit bin in % of the cells of its window
+                                       (266 time rows x npads): 0 = default 50, else 1..100.
+                                       100 can never overflow (D2: one digit per cell); the
+                                       densest config (C4) fills 35 %.  The digit bins are
+                                       most of the context's memory: 4 bytes x pct/100 x
+                                       1.04 x cells of the largest fragment    */
+  uint32_t reserved_;               /* must be 0                                               */
 } tpcclus_geometry;
 
 typedef struct {

@@ -22,9 +22,10 @@ TPCCLUS_ERR_CAPACITY = -3
 TPCCLUS_ERR_DIGIT = -4
 TPCCLUS_ERR_CUDA = -5
 TPCCLUS_ERR_NOMEM = -6
+TPCCLUS_ERR_OCCUPANCY = -7
 
 TPCCLUS_FLAG_EDGE_PAD, TPCCLUS_FLAG_EDGE_TIME, TPCCLUS_FLAG_SATURATED, TPCCLUS_FLAG_SPLIT = 1, 2, 4, 8
-TPCCLUS_OPT_STRICT_DIGITS, TPCCLUS_OPT_HOST_STAGING = 1, 2
+TPCCLUS_OPT_STRICT_DIGITS, TPCCLUS_OPT_HOST_STAGING, TPCCLUS_OPT_BIN_DIRECT = 1, 2, 4
 
 # record layouts of include/tpcclus.h
 DIGIT_DTYPE = np.dtype([("row", "u1"), ("pad", "u1"), ("time", "<u2"), ("charge", "<f4")])
@@ -44,7 +45,8 @@ class tpcclus_geometry(ctypes.Structure):
                 ("tf_time_bins", ctypes.c_uint32), ("max_core_bins", ctypes.c_uint32),
                 ("halo_bins", ctypes.c_uint32),
                 ("peak_min_q16", ctypes.c_uint16), ("options", ctypes.c_uint16),
-                ("max_digits", ctypes.c_uint64), ("max_clusters", ctypes.c_uint64)]
+                ("max_digits", ctypes.c_uint64), ("max_clusters", ctypes.c_uint64),
+                ("bin_occupancy_pct", ctypes.c_uint32), ("reserved_", ctypes.c_uint32)]
 
 
 class tpcclus_run_stats(ctypes.Structure):
@@ -110,7 +112,7 @@ def tpcclus_strerror(code: int) -> str:
 
 
 def tpcclus_create(npads, *, n_sectors, tf_time_bins, max_core_bins=None, halo_bins=0, peak_min_q16=64,
-                   options=0, max_digits, max_clusters=0, cuda_device=0):
+                   options=0, max_digits, max_clusters=0, bin_occupancy_pct=0, cuda_device=0):
     """tpcclus_create(geometry, device) -> opaque context handle (int)."""
     npads = np.ascontiguousarray(npads, dtype=np.uint16)
     g = tpcclus_geometry()
@@ -120,6 +122,7 @@ def tpcclus_create(npads, *, n_sectors, tf_time_bins, max_core_bins=None, halo_b
     g.max_core_bins = int(tf_time_bins if max_core_bins is None else max_core_bins)
     g.halo_bins, g.peak_min_q16, g.options = int(halo_bins), int(peak_min_q16), int(options)
     g.max_digits, g.max_clusters = int(max_digits), int(max_clusters)
+    g.bin_occupancy_pct, g.reserved_ = int(bin_occupancy_pct), 0
     h = ctypes.c_void_p()
     rc = lib().tpcclus_create(ctypes.byref(g), int(cuda_device), ctypes.byref(h))
     if rc != TPCCLUS_OK:

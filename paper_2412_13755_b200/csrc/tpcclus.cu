@@ -57,8 +57,6 @@ struct tpcclus_ctx {
   bool profiling = false;
   double prof_ms[TPCCLUS_N_KERNELS] = {};
   uint64_t prof_runs = 0;
-  int sticky = TPCCLUS_OK;
-  int sticky_cuda = 0;
   // host staging (TPCCLUS_OPT_HOST_STAGING)
   tpcclus_digit* d_stage_digits[2] = {nullptr, nullptr};
   tpcclus_cluster* d_stage_out[2] = {nullptr, nullptr};
@@ -70,40 +68,37 @@ namespace {
 
 inline uint32_t roundup(uint32_t x, uint32_t m) { return (x + m - 1) / m * m; }
 
-int cuda_fail(tpcclus_ctx* c, cudaError_t e) {
-  if (c) { c->sticky = TPCCLUS_ERR_CUDA; c->sticky_cuda = int(e); }
-  return TPCCLUS_ERR_CUDA;
-}
-
-// TPCCLUS_DEBUG=1 in the environment: synchronise after every launch and name the kernel that
-// failed on stderr (debugging aid; never set in tests or the bench).
-bool debug_sync() {
-  static const bool on = [] { const char* v = std::getenv("TPCCLUS_DEBUG"); return v && v[0] == '1'; }();
-  return on;
-}
+// Debugging aid, compiled in only with -DTPCCLUS_DEBUG_SYNC: synchronise after every launch and name the
+// kernel that failed on stderr.  The library reads no environment variables.
+#ifdef TPCCLUS_DEBUG_SYNC
 void debug_check(cudaStream_t st, const char* what) {
-  if (!debug_sync()) return;
   cudaError_t e = cudaStreamSynchronize(st);
   if (e == cudaSuccess) e = cudaGetLastError();
   std::fprintf(stderr, "[tpcclus] %s: %s\n", what, cudaGetErrorString(e));
 }
+#else
+inline void debug_check(cudaStream_t, const char*) {}
+#endif
 
 #define CK(ctx, call)                                  \
   do {                                                 \
     cudaError_t e__ = (call);                          \
-    if (e__ != cudaSuccess) return cuda_fail(ctx, e__); \
+    if (e__ != cudaSuccess) return TPCCLUS_ERR_CUDA;    \
   } while (0)
 
 template <typename T>
 int dev_alloc(tpcclus_ctx* c, T** p, uint64_t bytes) {
   cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes ? bytes : 16);
   if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return TPCCLUS_ERR_NOMEM; }
-  if (e != cudaSuccess) return cuda_fail(c, e);
+  if (e != cudaSuccess) return TPCCLUS_ERR_CUDA;
   c->dev_bytes += bytes;
   return TPCCLUS_OK;
 }
 
 }  // namespace
+
+static int run_tf_host_enqueue(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf, tpcclus_cluster* h_out,
+                               uint64_t cap, tpcclus_run_stats* stats);
 
 extern "C" {
 
@@ -116,6 +111,7 @@ const char* tpcclus_strerror(int code) {
     case TPCCLUS_ERR_DIGIT: return "invalid digit in strict mode";
     case TPCCLUS_ERR_CUDA: return "CUDA error";
     case TPCCLUS_ERR_NOMEM: return "out of memory";
+    case TPCCLUS_ERR_OCCUPANCY: return "digit bin overflow (bin_occupancy_pct too small for this input)";
     default: return "unknown status";
   }
 }
@@ -147,9 +143,10 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (!g || !out || !g->npads) return TPCCLUS_ERR_INVALID;
   *out = nullptr;
   if (g->n_sectors < 1 || g->n_sectors > (uint32_t)kMaxSectors || g->n_rows < 1 || g->n_rows > 256 ||
-      g->tf_time_bins < 1 || g->tf_time_bins > 65536 || g->max_core_bins < 1 ||
+      g->tf_time_bins < 1 || g->tf_time_bins > TPCCLUS_MAX_TF_BINS || g->max_core_bins < 1 ||
       g->max_core_bins > g->tf_time_bins || (g->halo_bins >= 1 && g->halo_bins < TPCCLUS_MIN_HALO) ||
-      g->halo_bins > 4096 || g->peak_min_q16 < 1 || g->peak_min_q16 > TPCCLUS_QMAX_Q16)
+      g->halo_bins > 4096 || g->peak_min_q16 < 1 || g->peak_min_q16 > TPCCLUS_QMAX_Q16 ||
+      g->bin_occupancy_pct > 100 || g->reserved_ != 0)
     return TPCCLUS_ERR_GEOMETRY;
   for (uint32_t r = 0; r < g->n_rows; ++r)
     if (g->npads[r] < 1 || g->npads[r] > TPCCLUS_MAX_NPADS) return TPCCLUS_ERR_GEOMETRY;
@@ -169,13 +166,15 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   if (prop.major < 10) return fail(TPCCLUS_ERR_CUDA);       // TMA + sm_100a code only; no fallback
   c->n_sm = prop.multiProcessorCount;
 
-  // geometry tables: one digit bin per (sector, row, kBinT time bins).  Capacity: 5/4 slots per
-  // cell of the bin's window (D2: at most one digit per cell; the rest absorbs the zero padding of
-  // k_bin's whole-sector flushes: < 16 entries per CTA and bin, and 7 per reserve-8 append)
+  // geometry tables: one digit bin per (sector, row, kBinT time bins).  Capacity: bin_occupancy_pct of the
+  // cells of the bin's window (D2: at most one digit per cell, so 100 % cannot overflow) plus what k_bin's
+  // whole-sector flushes pad with zero entries: at most 8 per bin for every CTA that works on the sector.
+  // A bin that receives more than its capacity makes the run fail with TPCCLUS_ERR_OCCUPANCY.
   c->tiles_per_row_max = (g->max_core_bins + kTileT - 1) / kTileT;
   c->bins_per_row_max = (g->max_core_bins + kBinT - 1) / kBinT;
   const uint32_t bin_rows = std::min<uint32_t>(uint32_t(kBinBoxH), g->max_core_bins + 2 * g->halo_bins);
-  const uint32_t cap_margin = 16u * uint32_t(c->n_sm) + 64u;
+  const uint32_t occ_pct = g->bin_occupancy_pct ? g->bin_occupancy_pct : 50u;
+  const uint32_t cap_margin = 8u * uint32_t(c->n_sm) + 64u;
   c->rows.resize(g->n_rows);
   uint64_t off = 0;
   uint32_t max_W = 0, max_npads = 0;
@@ -183,7 +182,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     RowInfo& ri = c->rows[r];
     ri.npads = c->npads[r];
     ri.W = uint16_t(roundup(ri.npads + 2 * kColOff, 8));
-    ri.cap = roundup(bin_rows * ri.npads + bin_rows * ri.npads / 4 + cap_margin, 8);
+    ri.cap = roundup((bin_rows * ri.npads * occ_pct + 99u) / 100u + cap_margin, 8);
     ri.ns = uint16_t(ri.W / 8);
     ri.fpb = uint16_t(flag_pitch_bytes(ri.W));
     {
@@ -197,9 +196,9 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
       ri.rcp_ns = (65536u + ri.ns - 1u) / ri.ns;
     }
     ri.pad_[0] = ri.pad_[1] = 0;
-    if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);
     ri.list_off = uint32_t(off);
     off += uint64_t(c->bins_per_row_max) * ri.cap;
+    if (off > 0xFFFFFFFFull) return fail(TPCCLUS_ERR_GEOMETRY);   // list offsets inside a sector are 32-bit
     max_W = std::max<uint32_t>(max_W, ri.W);
     max_npads = std::max<uint32_t>(max_npads, ri.npads);
   }
@@ -226,6 +225,9 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
     for (int k = 0; k <= TPCCLUS_N_KERNELS; ++k)
       if (cudaEventCreate(&c->ev_prof[i][k]) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
   }
+  // the bins start out as all "no digit" entries: whatever a later run leaves in slots it reserved but could
+  // not fill is then either zero or a well-formed entry of this geometry (memory safety for duplicate cells)
+  if (cudaMemset(c->d_lists, 0, list_bytes ? list_bytes : 16) != cudaSuccess) return fail(TPCCLUS_ERR_CUDA);
   if (cudaMemcpy(c->d_rows, c->rows.data(), g->n_rows * sizeof(RowInfo), cudaMemcpyHostToDevice) != cudaSuccess ||
       cudaMemset(c->d_tile_state, 0, uint64_t(c->max_tiles) * 8) != cudaSuccess ||
       cudaMemset(c->d_status, 0, sizeof(DevStatus)) != cudaSuccess)
@@ -243,7 +245,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
   {
     const uint32_t nb_max = g->n_rows * c->bins_per_row_max;
     c->bin_aggregated = nb_max <= kBinMaxNb && bin_smem_bytes(nb_max) <= uint32_t(prop.sharedMemPerBlockOptin) &&
-                        !std::getenv("TPCCLUS_BIN_DIRECT");
+                        !(g->options & TPCCLUS_OPT_BIN_DIRECT);
     if (c->bin_aggregated &&
         cudaFuncSetAttribute(k_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, int(prop.sharedMemPerBlockOptin)) != cudaSuccess)
       return fail(TPCCLUS_ERR_CUDA);
@@ -251,7 +253,7 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
       int bocc = 0;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bocc, k_bin, kBinThreads, bin_smem_bytes(nb_max)) != cudaSuccess || bocc < 1)
         return fail(TPCCLUS_ERR_CUDA);
-      c->bin_ctas_per_sm = bocc;
+      c->bin_ctas_per_sm = 1;   // the bins' capacity margin (8 slots per CTA and bin) is sized for one CTA per SM
     }
   }
 
@@ -416,6 +418,7 @@ int tpcclus_result(tpcclus_ctx* c, tpcclus_run_stats* stats) {
   stats->n_clusters = c->h_status[slot].n_clusters;
   int rc = TPCCLUS_OK;
   if ((c->g.options & TPCCLUS_OPT_STRICT_DIGITS) && stats->n_digits_dropped) rc = TPCCLUS_ERR_DIGIT;
+  else if (c->h_status[slot].n_overfull_bins) rc = TPCCLUS_ERR_OCCUPANCY;
   else if (stats->n_clusters > c->pending[slot].cap) rc = TPCCLUS_ERR_CAPACITY;
   stats->status = rc;
   return rc;
@@ -439,9 +442,37 @@ int tpcclus_run_tf_host(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf,
                         uint64_t cap, tpcclus_run_stats* stats) {
   if (!c || !fr || !stats || nf == 0 || (cap && !h_out) || c->head != c->tail) return TPCCLUS_ERR_INVALID;
   if (!(c->g.options & TPCCLUS_OPT_HOST_STAGING)) return TPCCLUS_ERR_INVALID;
-  for (uint32_t f = 0; f < nf; ++f)
-    if (fr[f].n > c->g.max_digits || (fr[f].n && !fr[f].h_digits) || !fr[f].h_sector_offsets) return TPCCLUS_ERR_INVALID;
+  // every fragment is validated before anything is enqueued, so that no copy is in flight when an argument
+  // error is reported
+  for (uint32_t f = 0; f < nf; ++f) {
+    const tpcclus_fragment& x = fr[f];
+    if (x.n > c->g.max_digits || (x.n && !x.h_digits) || !x.h_sector_offsets) return TPCCLUS_ERR_INVALID;
+    if (!(x.t_core_begin < x.t_core_end) || x.t_core_end > c->g.tf_time_bins ||
+        x.t_core_end - x.t_core_begin > c->g.max_core_bins)
+      return TPCCLUS_ERR_INVALID;
+    if (x.h_sector_offsets[0] != 0 || x.h_sector_offsets[c->g.n_sectors] != x.n) return TPCCLUS_ERR_INVALID;
+    for (uint32_t s2 = 0; s2 < c->g.n_sectors; ++s2)
+      if (x.h_sector_offsets[s2 + 1] < x.h_sector_offsets[s2]) return TPCCLUS_ERR_INVALID;
+  }
   CK(c, cudaSetDevice(c->device));
+  for (uint32_t f = 0; f < nf; ++f) {
+    std::memset(&stats[f], 0, sizeof(stats[f]));
+    stats[f].status = TPCCLUS_ERR_INVALID;                  // "not run" until the fragment has been reported
+  }
+  const int rc_tf = run_tf_host_enqueue(c, fr, nf, h_out, cap, stats);
+  // whatever happened, nothing of this call may still be reading the caller's buffers or writing h_out
+  const cudaError_t e1 = cudaStreamSynchronize(c->s_h2d), e2 = cudaStreamSynchronize(c->s_run),
+                    e3 = cudaStreamSynchronize(c->s_d2h);
+  while (c->head != c->tail) { tpcclus_run_stats drop; tpcclus_result(c, &drop); }   // (only after an error)
+  if (rc_tf == TPCCLUS_OK && (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess)) return TPCCLUS_ERR_CUDA;
+  return rc_tf;
+}
+
+}  // extern "C"
+
+// The pipeline proper; the caller synchronises the three streams afterwards on every path.
+static int run_tf_host_enqueue(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf, tpcclus_cluster* h_out,
+                               uint64_t cap, tpcclus_run_stats* stats) {
   int first_err = TPCCLUS_OK;
   uint64_t written = 0;
   // prologue: H2D of fragment 0
@@ -480,10 +511,10 @@ int tpcclus_run_tf_host(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf,
     CK(c, cudaEventRecord(c->ev_d2h[slot], c->s_d2h));
     written += ncopy;
   }
-  CK(c, cudaStreamSynchronize(c->s_d2h));
-  CK(c, cudaStreamSynchronize(c->s_h2d));
   return first_err;
 }
+
+extern "C" {
 
 int tpcclus_run_host(tpcclus_ctx* c, const tpcclus_digit* h_digits, uint64_t n, const uint64_t* h_off, uint32_t b,
                      uint32_t e, tpcclus_cluster* h_out, uint64_t cap, tpcclus_run_stats* stats) {

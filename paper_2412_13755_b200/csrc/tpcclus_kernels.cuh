@@ -6,15 +6,15 @@
 //                                     packed 4-byte entry in the list of every (sector,row,256-bin) digit
 //                                     bin whose window holds it; write-combined: one 32-byte sector and
 //                                     one global atomic per 8 entries
-//                            k_tile   front warps: the bin's list is scattered into the (pad x time)
-//                                     charge map of the tile, which lives in shared memory only
-//   S2  peak finding         k_tile   front warps: digit-driven 3x3 ordered-maximum test on the smem map
-//                                     -> flag bitmap; then each peak's 80-byte window is cut out
-//   S3  peak count S(c)      k_tile   back warps: other peaks of the 9x9 flag window, table-driven
-//   S4  5x5 assembly         k_tile   back warps: four lanes per peak (rotation classes)
-//   S5  centroid / width     k_tile   back warps: exact integer moments; committer warp: fp64 finish
-//   S6  ordered compaction   k_tile   front warps: popc prefix inside the tile; committer warp: decoupled
-//                                     look-back across tiles in (sector,row,time) ticket order, copy-out
+//                            k_tile   the bin's list is scattered into the (pad x time) charge map of the
+//                                     tile, which lives in shared memory only                (tpcclus_tile.cuh)
+//   S2  peak finding         k_tile   dense packed-u16x2 sweep of the map -> one flag byte per 8 cells
+//   S3  peak count S(c)      k_tile   one thread per peak: other peaks of the 9x9 flag window, table-driven
+//   S4  5x5 assembly         k_tile   one thread per peak, 25 charges straight from the map
+//   S5  centroid / width     k_tile   exact integer moments from column / row weight sums; committer warp:
+//                                     fp64 finish
+//   S6  ordered compaction   k_tile   popc prefix inside the tile; committer warp: decoupled look-back across
+//                                     tiles in (sector,row,time) ticket order, copy-out
 //   S7  fragment ownership   k_tile   tiles cover exactly the core [b,e); halo rows never emit
 //
 // Definitions D1..D12 are those of SURVEY.md §8(c) (restated in DESIGN.md §2); the D-number
@@ -47,7 +47,7 @@ constexpr int      kMaxSectors   = 256;
 
 struct RowInfo {              // one per pad row (device table), 32 bytes
   uint32_t list_off;          // element offset of this row's bins inside one sector's digit lists
-  uint32_t cap;               // list capacity of one bin (multiple of 8): window cells * 5/4 + padding margin
+  uint32_t cap;               // list capacity of one bin (multiple of 8): bin_occupancy_pct of the window's cells + padding margin
   uint16_t npads;
   uint16_t W;                 // smem map pitch in cells = roundup8(npads + 4)
   // k_tile's sweep over a tile of this row: strips of 8 cells x row segments
@@ -64,7 +64,7 @@ struct DevStatus {            // device-side run status, copied to pinned host m
   unsigned long long n_dropped;
   unsigned long long n_clusters;
   unsigned int       ticket;  // tile ticket counter of k_tile
-  unsigned int       pad_;
+  unsigned int       n_overfull_bins;   // digit bins that received more entries than their capacity
 };
 
 struct BinParams {
@@ -172,6 +172,7 @@ __global__ void __launch_bounds__(256) k_init(uint32_t* __restrict__ counts, uin
     status->n_dropped = 0ull;
     status->n_clusters = 0ull;
     status->ticket = 0u;
+    status->n_overfull_bins = 0u;
   }
   const uint32_t n4 = (n_tiles + 3u) >> 2;                 // the array is padded to a multiple of 4
   for (uint32_t k = i; k < n4; k += gridDim.x * blockDim.x)
@@ -181,13 +182,12 @@ __global__ void __launch_bounds__(256) k_init(uint32_t* __restrict__ counts, uin
 // ----------------------------------------------------------------------------------------
 // S1 (first half): digit binning.  One 16-byte load = two digits (BASELINE.json:north_star (2):
 // "16-byte vectorised coalesced loads").  D1 quantisation; invalid digits dropped and counted.
-// A valid digit at global time t is appended, as pad | tl<<8 | q16<<16 with tl its row inside
-// the tile's 138-row window, to the list of every tile tt whose window
-// [b + 128 tt - 5, b + 128 tt + 133) contains t (one tile, or two next to a tile seam).
-// A bin has one slot per map cell, so it cannot overflow while D2's precondition (at most one
-// digit per cell) holds; slots past the capacity are discarded (memory-safe for duplicates).
+// A valid digit at global time t is appended, as a packed entry with tl = its row inside the
+// bin's 266-row window, to the list of every bin tb whose window [b + 256 tb - 5, b + 256 tb + 261)
+// contains t (one bin, or two next to a bin seam).  Entries past a bin's capacity are discarded
+// (memory-safe for duplicate cells) and the bin is reported (TPCCLUS_ERR_OCCUPANCY).
 // ----------------------------------------------------------------------------------------
-// packed list entry: pad (8 bits) | tl << 8 (row of the tile window, 9 bits) | q16 << 17 (14 bits)
+// packed list entry: pad (8 bits) | tl << 8 (row of the bin's window, 9 bits) | q16 << 17 (14 bits)
 __device__ __forceinline__ uint32_t pack_digit(uint32_t pad, uint32_t tl, uint32_t q) { return pad | (tl << 8) | (q << 17); }
 __device__ __forceinline__ uint32_t dig_pad(uint32_t d) { return d & 0xFFu; }
 __device__ __forceinline__ uint32_t dig_tl(uint32_t d) { return (d >> 8) & 0x1FFu; }
@@ -199,9 +199,8 @@ __device__ __forceinline__ uint32_t quantise_q16(float charge) {
   return min(__float2uint_rn(charge * 16.0f), kQClamp);
 }
 
-// append one packed digit to a bin, reserving R slots (R = 1: k_bin_direct; R = 8: the odd
-// entries of the write-combining kernel, whose reservations stay multiples of 8 — the other
-// R-1 slots are zero = "no digit")
+// append one packed digit to a bin, reserving R slots (R = 1 everywhere now; the other R-1 slots
+// would be zero = "no digit")
 template <int R>
 __device__ __forceinline__ void bin_append(uint32_t* __restrict__ seclist, uint32_t* __restrict__ cnt, uint32_t dest0,
                                            uint32_t cap, uint32_t pk) {
@@ -307,7 +306,6 @@ constexpr int      kBinChunk    = kBinThreads * kBinPer;    // 6144 digits = 48 
 constexpr int      kBinSecCap   = 1024;                     // second (seam) entries kept per chunk
 constexpr uint32_t kBinMaxNb    = 4096;                     // bins per sector (12-bit bin id)
 constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room (duplicates only)
-constexpr uint32_t kBinNone     = 0xFFFFFFFFu;              // staging slot without a list entry
 
 __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
   const uint32_t nb4 = (nb + 3u) & ~3u;
@@ -315,7 +313,18 @@ __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
          3u * 256u * 4u + 96u + 128u;
 }
 
-__device__ __forceinline__ void st_v4(uint32_t* p, uint4 v) { *reinterpret_cast<uint4*>(p) = v; }
+// store a bin buffer (8 entries) at list position p: one aligned 32-byte sector on the production path; the
+// reservations stop being multiples of 8 only after a single-entry append (second entries beyond kBinSecCap,
+// i.e. time-sorted input), and then the entries go out one by one
+__device__ __forceinline__ void store8(uint32_t* p, uint4 a, uint4 c) {
+  if ((reinterpret_cast<uintptr_t>(p) & 15u) == 0u) {
+    *reinterpret_cast<uint4*>(p) = a;
+    *reinterpret_cast<uint4*>(p + 4) = c;
+  } else {
+    p[0] = a.x; p[1] = a.y; p[2] = a.z; p[3] = a.w;
+    p[4] = c.x; p[5] = c.y; p[6] = c.z; p[7] = c.w;
+  }
+}
 
 __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ BinParams P,
                                                         const RowInfo* __restrict__ rows, uint32_t* __restrict__ lists,
@@ -368,7 +377,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     for (int k = 0; k < ne; ++k) {
       uint32_t s0 = 0;
       const uint2 v = dg[edge[k]];
-      dropped += bin_one<8>(v.x, v.y, edge[k], s0, P, rows, lists, counts) ? 0u : 1u;
+      dropped += bin_one<1>(v.x, v.y, edge[k], s0, P, rows, lists, counts) ? 0u : 1u;
     }
   }
 
@@ -445,8 +454,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
         const uint32_t d = nxt[bin];
         if (d != kBinFull) {
-          st_v4(seclist + d, a);
-          st_v4(seclist + d + 4, c);
+          store8(seclist + d, a, c);
         }
         cnt[bin] = 0u;
       }
@@ -530,9 +538,9 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
                 const uint32_t k2 = atomicAdd(nsecp, 1u);
                 if (k2 < uint32_t(kBinSecCap)) {
                   sec[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
-                } else {                                      // second-entry list full: reserve-8 direct path
+                } else {                                      // second-entry list full: direct path
                   const uint32_t cap = r_cap[row];
-                  bin_append<8>(seclist, &counts[cbase + bin + 1u], r_off[row] + uint32_t(tlo + 1) * cap, cap, pk2);
+                  bin_append<1>(seclist, &counts[cbase + bin + 1u], r_off[row] + uint32_t(tlo + 1) * cap, cap, pk2);
                 }
               }
             }
@@ -555,8 +563,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
         const uint32_t d = nxt[bin];
         if (d != kBinFull) {
-          st_v4(seclist + d, a);
-          st_v4(seclist + d + 4, c);
+          store8(seclist + d, a, c);
         }
         res_g[x] = atomicAdd(&counts[cbase + bin], 8u);       // the next sector, looked at one chunk later
         res_m |= 1u << x;

@@ -406,6 +406,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     s_next[1] = sector | (row << 8);
     s_next[2] = tt;
     s_next[3] = min(count, cap);                                          // k_bin: a multiple of 8; 0 entries are padding
+    if (count > cap) atomicAdd(&P.status->n_overfull_bins, 1u);           // -> TPCCLUS_ERR_OCCUPANCY
     s_next[4] = uint32_t(src);
     s_next[5] = uint32_t(src >> 32);
   };

@@ -18,14 +18,15 @@ class GpuClusterizer:
     """One context; run(...) returns the records as a numpy structured array."""
 
     def __init__(self, npads, *, n_sectors, tf_time_bins, max_core_bins=None, halo_bins=0, peak_min_q16=64,
-                 max_digits, options=0, max_clusters=0):
+                 max_digits, options=0, max_clusters=0, bin_occupancy_pct=0):
         import paper_2412_13755_b200 as T
 
         self.T = T
         self.ctx = T.tpcclus_create(npads, n_sectors=n_sectors, tf_time_bins=tf_time_bins,
                                     max_core_bins=max_core_bins, halo_bins=halo_bins,
                                     peak_min_q16=peak_min_q16, options=options,
-                                    max_digits=max(int(max_digits), 1), max_clusters=max_clusters)
+                                    max_digits=max(int(max_digits), 1), max_clusters=max_clusters,
+                                    bin_occupancy_pct=bin_occupancy_pct)
 
     def close(self):
         if self.ctx:
@@ -60,13 +61,14 @@ class GpuClusterizer:
 
 
 def gpu_clusters(digits, offs, npads, *, n_sectors, tf_time_bins, t_core_begin=0, t_core_end=None, halo_bins=0,
-                 peak_min_q16=64):
+                 peak_min_q16=64, options=0, bin_occupancy_pct=0):
     if t_core_end is None:
         t_core_end = tf_time_bins
     d = to_device_digits(digits)
     with GpuClusterizer(npads, n_sectors=n_sectors, tf_time_bins=tf_time_bins,
                         max_core_bins=t_core_end - t_core_begin, halo_bins=halo_bins,
-                        peak_min_q16=peak_min_q16, max_digits=d.shape[0]) as g:
+                        peak_min_q16=peak_min_q16, max_digits=d.shape[0], options=options,
+                        bin_occupancy_pct=bin_occupancy_pct) as g:
         return g.run(d, offs, t_core_begin, t_core_end)
 
 

@@ -35,7 +35,7 @@ def test_library_builds_loads_and_exports_every_symbol():
 def test_record_layouts_match_header():
     import paper_2412_13755_b200 as T
 
-    assert ctypes.sizeof(T.tpcclus_geometry) == 48
+    assert ctypes.sizeof(T.tpcclus_geometry) == 56
     assert ctypes.sizeof(T.tpcclus_run_stats) == 32
     assert ctypes.sizeof(T.tpcclus_fragment) == 32
     assert T.CLUSTER_DTYPE.fields["time"][1] == 4 and T.CLUSTER_DTYPE.fields["qtot"][1] == 12
@@ -68,3 +68,12 @@ def test_product_does_not_import_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2412_13755_b200" not in txt and "from paper_2412_13755_b200" not in txt
             assert "#include \"../include" not in txt and "#include \"tpcclus" not in txt
+
+
+def test_product_reads_no_environment_variables():
+    """behaviour is selected by the geometry struct only — no env vars, no global state."""
+    pkg = os.path.join(ROOT, "paper_2412_13755_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".cu", ".cuh", ".h")):
+                assert "getenv" not in open(os.path.join(dirpath, f)).read(), f

@@ -49,3 +49,19 @@ def test_single_rank_is_identity():
     import bench
 
     assert bench.dist_max_sum(3.5, 7.0, 1) == (3.5, 7.0)
+
+
+def test_bare_gpus_flag_launches_the_ranks_itself():
+    """`python bench.py --gpus 2` without torchrun's environment starts the two ranks itself (one process per
+    GPU through torch.distributed.run on 127.0.0.1).  Exercised on CPU with the reference arm (rank 0 times the
+    oracle on config 0 and prints the line, rank 1 exits 0 without work)."""
+    import json
+
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference",
+                        "--config", "0", "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True,
+                       timeout=600)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [json.loads(x) for x in p.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+    assert lines[0]["value"] > 0 and lines[0]["cpu_baseline"]["kind"] == "oracle"

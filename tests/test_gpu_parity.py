@@ -307,17 +307,159 @@ def test_unaligned_digit_buffer_and_sector_seams():
         assert got.tobytes() == ref.tobytes(), shift
 
 
-def test_direct_binning_fallback_matches(monkeypatch):
+def test_direct_binning_fallback_matches():
     """k_bin_direct (taken when a geometry's bins do not fit the write-combining kernel's shared
-    memory; forced here with TPCCLUS_BIN_DIRECT=1) gives the same bytes."""
+    memory; forced here with TPCCLUS_OPT_BIN_DIRECT) gives the same bytes."""
+    import paper_2412_13755_b200 as T
+
     cfg = gen.config("c4mini", tf_time_bins=300, core_bins=300)
     d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
     dn = gen.as_numpy_digits(d)
     kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
     a, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
-    monkeypatch.setenv("TPCCLUS_BIN_DIRECT", "1")
-    b, _ = gpu_clusters(dn, offs, cfg.npads_array(), **kw)
-    assert len(a) > 1e4 and a.tobytes() == b.tobytes()
+    b, _ = gpu_clusters(dn, offs, cfg.npads_array(), options=T.TPCCLUS_OPT_BIN_DIRECT, **kw)
+    ref, _ = oracle.run(dn, offs, cfg.npads_array(), **kw)
+    assert len(a) > 1e4 and a.tobytes() == b.tobytes() == ref.tobytes()
+
+
+def test_bin_occupancy_sizing_and_overflow_error():
+    """The digit bins are sized from geometry.bin_occupancy_pct (scratch is sized ahead with a
+    safety margin).  100 % can never overflow; the default (50 %) holds the 35 % stress config; a context sized
+    for 2 % reports TPCCLUS_ERR_OCCUPANCY on it — a defined error, not a fault — and works again on sparse input."""
+    import paper_2412_13755_b200 as T
+
+    cfg = gen.config("c4mini", tf_time_bins=600, core_bins=600)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    npads = cfg.npads_array()
+    kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    ref, _ = oracle.run(dn, offs, npads, **kw)
+    sizes = {}
+    for pct in (0, 100, 40):
+        with GpuClusterizer(npads, max_digits=len(dn), bin_occupancy_pct=pct, **kw) as g:
+            got, st = g.run(d, offs, 0, cfg.tf_time_bins)
+            sizes[pct] = T.tpcclus_device_bytes(g.ctx)
+        assert st["status"] == 0 and got.tobytes() == ref.tobytes(), pct
+    assert sizes[40] < sizes[0] < sizes[100]
+    sparse, so = digits_from_cells([(0, 3, 5, 17, 30.0), (1, 9, 2, 400, 9.0)], n_sectors=2)
+    with GpuClusterizer(npads, max_digits=len(dn), bin_occupancy_pct=2, **kw) as g:
+        _, st = g.run(d, offs, 0, cfg.tf_time_bins, capacity=len(ref), check=False)
+        assert st["status"] == T.TPCCLUS_ERR_OCCUPANCY and st["cuda_error"] == 0
+        got, st = g.run(to_device_digits(sparse), so, 0, cfg.tf_time_bins)
+        want, _ = oracle.run(sparse, so, npads, **kw)
+        assert st["status"] == 0 and len(want) == 2 and got.tobytes() == want.tobytes()
+    with pytest.raises(T.TpcclusError) as ei:
+        T.tpcclus_create(npads, max_digits=10, bin_occupancy_pct=101, **kw)
+    assert ei.value.code == T.TPCCLUS_ERR_GEOMETRY
+
+
+@pytest.mark.parametrize("name,rows", [(0, [0, 77, 151]), ("c4mini", [0, 40, 151]), ("c3mini", [3, 100])])
+def test_peak_flags_cell_by_cell(name, rows):
+    """BJ:north_star: "peak flags ... must be bit-exact against the oracle".  The library emits exactly one record
+    per peak of the core (D10), so its D4 flag map is the set of its records' (time, pad): rebuilt per
+    (sector,row) and fragment and compared cell by cell with tpc_oracle_peak_flags (the oracle's steps 1-2)."""
+    cfg = gen.config(name)
+    npads = cfg.npads_array()
+    with GpuClusterizer(npads, n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins, max_core_bins=cfg.core_bins,
+                        halo_bins=cfg.halo_bins, max_digits=1 << 28) as g:
+        for f, (b, e) in enumerate(cfg.fragments()):
+            d, offs, _ = gen.generate_fragment(cfg, f, device="cuda")
+            got, _ = g.run(d, offs, b, e)
+            dn = gen.as_numpy_digits(d)
+            lo = max(0, b - cfg.halo_bins)
+            n_flags = 0
+            for s in range(cfg.n_sectors):
+                for r in rows:
+                    want, _q = oracle.peak_flags(dn, offs, npads, n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins,
+                                                 sector=s, row=r, t_core_begin=b, t_core_end=e, halo_bins=cfg.halo_bins)
+                    want = want[b - lo: e - lo]                          # D9: only the core's peaks emit
+                    mine = np.zeros_like(want)
+                    k = got[(got["sector"] == s) & (got["row"] == r)]
+                    assert np.all((k["time"] >= b) & (k["time"] < e))
+                    mine[k["time"].astype(np.int64) - b, k["pad"]] = 1
+                    assert int(mine.sum()) == len(k)                      # no two records on one cell
+                    assert np.array_equal(mine, want != 0), (f, s, r)
+                    n_flags += int(mine.sum())
+            assert n_flags > 50
+
+
+def _d1_fuzz_charges(rng, n):
+    """float32 charges that exercise every branch of D1: half-way cases of the 1/16 grid (round-half-even), values
+    one ulp either side of them, the ZS / zero boundary 1/32, the clamp at 1023, negatives, -0.0, tiny and
+    subnormal values, infinities, NaN and huge values."""
+    f32 = np.float32
+    k = rng.integers(0, 16400, size=n)                                     # 16 * half = k + 0.5, up to just past the clamp
+    half = ((2 * k + 1) / 32.0).astype(f32)                                # exactly between two grid points
+    kind = rng.integers(0, 12, size=n)
+    out = np.empty(n, dtype=f32)
+    special = np.array([1e-30, -1e-30, -0.0, 0.0, -3.5, np.inf, -np.inf, np.nan, 1e-40, -1e-40, 5000.0, 3e38,
+                        1022.96875, 1023.0, 1023.03125, 16367.5 / 16, 16368.5 / 16, 1.0 / 32, 3.0 / 32, 0.5 / 16],
+                       dtype=f32)
+    near = np.array([1.0 / 32, 1023.0, 16367.5 / 16, 1022.96875, 0.09375, 2.0], dtype=f32)
+    for i in range(12):
+        m = kind == i
+        c = int(m.sum())
+        if i < 3:
+            out[m] = half[m]
+        elif i == 3:
+            out[m] = np.nextafter(half[m], f32(np.inf))
+        elif i == 4:
+            out[m] = np.nextafter(half[m], f32(-np.inf))
+        elif i == 5:
+            out[m] = rng.choice(special, size=c)
+        elif i == 6:
+            b = rng.choice(near, size=c)
+            steps = rng.integers(-3, 4, size=c)
+            v = b.copy()
+            for _ in range(3):
+                up = steps > 0
+                dn = steps < 0
+                v[up] = np.nextafter(v[up], f32(np.inf))
+                v[dn] = np.nextafter(v[dn], f32(-np.inf))
+                steps = steps - np.sign(steps)
+            out[m] = v
+        elif i == 7:
+            out[m] = rng.uniform(0.0, 40.0, size=c).astype(f32)            # off-grid ordinary values
+        elif i == 8:
+            out[m] = rng.uniform(1000.0, 1050.0, size=c).astype(f32)       # around the clamp
+        elif i == 9:
+            out[m] = rng.uniform(0.0, 0.2, size=c).astype(f32)             # around the zero boundary
+        elif i == 10:
+            out[m] = -rng.uniform(0.0, 10.0, size=c).astype(f32)
+        else:
+            out[m] = (rng.integers(32, 16368, size=c) / 16.0).astype(f32)  # on the grid
+    return out
+
+
+def test_d1_quantisation_fuzz_through_the_cuda_path():
+    """D1 on the CUDA path beyond the 1/16 grid: 1.3e6 digits on distinct cells whose charges hit the half-way
+    cases, both clamps, signs, infinities, NaN and subnormals; records and n_digits_dropped equal the oracle's
+    (whose quantiser is pinned against exact rationals in test_oracle_peakflags_d1.py).  The same input in
+    STRICT mode is the error TPCCLUS_ERR_DIGIT."""
+    import paper_2412_13755_b200 as T
+
+    rng = np.random.default_rng(77)
+    n_sectors, n_rows, w, nt, n = 2, 64, 128, 300, 1_300_000
+    cell = rng.choice(n_sectors * n_rows * w * nt, size=n, replace=False)
+    cell.sort()
+    d = np.zeros(n, dtype=oracle.DIGIT_DTYPE)
+    d["pad"] = cell % w
+    d["time"] = (cell // w) % nt
+    d["row"] = (cell // (w * nt)) % n_rows
+    sec = cell // (w * nt * n_rows)
+    d["charge"] = _d1_fuzz_charges(rng, n)
+    offs = np.searchsorted(sec, np.arange(n_sectors + 1)).astype(np.uint64)
+    d = permute_within_sectors(d, offs, rng)
+    npads = [w] * n_rows
+    for theta in (1, 64):
+        got, ref, st = both(d, offs, npads, n_sectors=n_sectors, tf_time_bins=nt, peak_min_q16=theta)
+        assert st["n_digits_dropped"] > 0.1 * n and len(ref) > 1e4
+        assert (ref["flags"] & 4).any()
+        assert got.tobytes() == ref.tobytes()
+    with GpuClusterizer(npads, n_sectors=n_sectors, tf_time_bins=nt, max_digits=n,
+                        options=T.TPCCLUS_OPT_STRICT_DIGITS) as g:
+        _, st = g.run(to_device_digits(d), offs, 0, nt, capacity=8, check=False)
+        assert st["status"] == T.TPCCLUS_ERR_DIGIT
 
 
 def _random_cells(rng, n_sectors, npads, t_lo, t_hi, n, max_q=400.0):
