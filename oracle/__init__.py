@@ -19,7 +19,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tpc_oracle.cpp")
-_LIB = os.path.join(_HERE, "libtpc_oracle.so")
+# TPC_ORACLE_SANITIZE=1: the checker itself built with -fsanitize=address,undefined, for
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) TPC_ORACLE_SANITIZE=1 python -m pytest tests -m "not gpu"
+_SANITIZE = os.environ.get("TPC_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "libtpc_oracle_san.so" if _SANITIZE else "libtpc_oracle.so")
 
 DIGIT_DTYPE = np.dtype(
     [("row", "u1"), ("pad", "u1"), ("time", "<u2"), ("charge", "<f4")], align=False
@@ -65,7 +68,9 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
         subprocess.check_call(
-            ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall", "-Wextra", _SRC, "-o", tmp]
+            ["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-Wall", "-Wextra",
+             *(["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+               if _SANITIZE else []), _SRC, "-o", tmp]
         )
         os.replace(tmp, _LIB)
     return _LIB

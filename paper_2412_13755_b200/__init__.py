@@ -71,6 +71,15 @@ class TpcclusError(RuntimeError):
 
 _lock = threading.Lock()
 _lib = None
+_checked = False
+
+
+def use_checked_build() -> None:
+    """Select csrc/libtpcclus_checked.so (same sources with -DTPCCLUS_CHECKED: device asserts on every shared-memory
+    and list index).  Must be called before the first use of the library; for tests/sanitizer_cases.py."""
+    global _checked
+    assert _lib is None, "the library is already loaded"
+    _checked = True
 
 
 def lib():
@@ -78,7 +87,7 @@ def lib():
     global _lib
     with _lock:
         if _lib is None:
-            L = ctypes.CDLL(_build.build())
+            L = ctypes.CDLL(_build.build(checked=_checked))
             vp, u64, u32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32
             L.tpcclus_create.restype = ctypes.c_int
             L.tpcclus_create.argtypes = [ctypes.POINTER(tpcclus_geometry), ctypes.c_int, ctypes.POINTER(vp)]

@@ -25,6 +25,16 @@
 #include <stdint.h>
 #include <type_traits>
 
+// -DTPCCLUS_CHECKED (paper_2412_13755_b200/build.py: build(checked=True) -> libtpcclus_checked.so): every
+// shared-memory and list index of the kernels is bounds-checked with a device assert.  This is the repo's own
+// stand-in for compute-sanitizer memcheck, which is closed on this GPU pool (profiles/r2_sanitizer.md).
+#ifdef TPCCLUS_CHECKED
+#include <cassert>
+#define TPC_ASSERT(x) assert(x)
+#else
+#define TPC_ASSERT(x) ((void)0)
+#endif
+
 namespace tpcclus {
 
 #ifndef TPCCLUS_TILE_T
@@ -206,6 +216,7 @@ __device__ __forceinline__ void bin_append(uint32_t* __restrict__ seclist, uint3
                                            uint32_t cap, uint32_t pk) {
   const uint32_t slot = atomicAdd(cnt, uint32_t(R));
   if (slot + uint32_t(R) <= cap) {
+    TPC_ASSERT(pk != 0u);
     seclist[dest0 + slot] = pk;
 #pragma unroll
     for (int x = 1; x < R; ++x) seclist[dest0 + slot + x] = 0u;
@@ -454,6 +465,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
         const uint32_t d = nxt[bin];
         if (d != kBinFull) {
+          TPC_ASSERT(n < 8u && d >= b_off[x] && d + 8u <= b_off[x] + b_cap[x] && uint64_t(d) + 8u <= P.sec_list_elems);
           store8(seclist + d, a, c);
         }
         cnt[bin] = 0u;
@@ -498,6 +510,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
 
     // rank an entry inside its bin; ranks 0..7 go to the bin's buffer
     auto insert = [&](uint32_t bin, uint32_t pk) -> uint32_t {
+      TPC_ASSERT(bin < P.nb && pk != 0u);
       const uint32_t r = atomicAdd(&cnt[bin], 1u);
       if (r < 8u) buf[bin * 8u + r] = pk;
       return r;
@@ -536,6 +549,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
               if (thi != tlo) {                               // also in the next bin's window
                 const uint32_t pk2 = pk - (uint32_t(kBinT) << 8);
                 const uint32_t k2 = atomicAdd(nsecp, 1u);
+                TPC_ASSERT(bin + 1u < P.nb && uint32_t(thi) == uint32_t(tlo) + 1u);
                 if (k2 < uint32_t(kBinSecCap)) {
                   sec[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
                 } else {                                      // second-entry list full: direct path
@@ -563,6 +577,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
         const uint32_t d = nxt[bin];
         if (d != kBinFull) {
+          TPC_ASSERT(d >= b_off[x] && d + 8u <= b_off[x] + b_cap[x] && uint64_t(d) + 8u <= P.sec_list_elems);
           store8(seclist + d, a, c);
         }
         res_g[x] = atomicAdd(&counts[cbase + bin], 8u);       // the next sector, looked at one chunk later
@@ -582,10 +597,13 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     auto place = [&](uint32_t pk, uint32_t y) {
       const uint32_t bin = y & 0xFFFu, r = y >> 12;
       const uint32_t nf8 = uint32_t(nfull[bin]) << 3;
+      TPC_ASSERT(bin < P.nb && r >= 8u);
       if (r >= nf8) {
+        TPC_ASSERT(r - nf8 < 8u);
         buf[bin * 8u + (r - nf8)] = pk;
       } else {
         const uint32_t d = dst[bin];
+        TPC_ASSERT(d == kBinFull || uint64_t(d) + r < P.sec_list_elems);
         if (d != kBinFull) seclist[d + r] = pk;
       }
     };

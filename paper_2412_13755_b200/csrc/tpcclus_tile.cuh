@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         excl = lookback_exclusive(P.tile_state, t, P.epoch, total);
         if (lane == 0 && t == P.n_tiles - 1) P.status->n_clusters = (unsigned long long)excl + total;
       }
+      TPC_ASSERT(cnt <= uint32_t(kListCap) && off + cnt <= total);
       const uint64_t g0 = uint64_t(excl) + off;                          // first record of this item
       const uint4* src = stage + b * (2u * kListCap);
       uint4* dst = reinterpret_cast<uint4*>(P.out) + 2 * g0;
@@ -441,6 +442,8 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     const uint32_t* fw = reinterpret_cast<const uint32_t*>(mapraw + kMapGuard + flag_off);
     const uint4* src4 = reinterpret_cast<const uint4*>(src);
     const uint32_t n4 = n >> 2;
+    TPC_ASSERT(n <= ri.cap && (reinterpret_cast<uintptr_t>(src) & 15u) == 0u && tt < P.tiles_per_row &&
+               flag_off + uint32_t(kBoxH) * fpb + uint32_t(kMapGuard) <= P.map_bytes_max);
 
     // ---- D2: zero the tile's charge map, the guard behind it and the flag bytes ----
     {
@@ -460,6 +463,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     {
       auto put = [&](uint32_t d) {
         const uint32_t tl = dig_tl(d);
+        TPC_ASSERT(d == 0u || (tl < uint32_t(kBoxH) && dig_pad(d) < ri.npads && dig_q(d) >= 1u && dig_q(d) <= kQClamp));
         if (d && tl < uint32_t(kBoxH)) map[tl * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
       };
       uint32_t i = tid;
@@ -495,6 +499,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
       const uint32_t nout = owner ? L : 0u;
       uint32_t a = map_s + jb * pitch + 16u * s;
       uint32_t f = flag_s + (jb + 1u) * fpb + 4u + s;
+      TPC_ASSERT(s < ns && 16u * s + 16u <= pitch && jb + L + 2u <= uint32_t(kBoxH) && 4u + s < fpb);
       SweepRow ra, rb;
       sweep_step<false, false>(a, theta2, ra, ra);
       a += pitch;
@@ -587,6 +592,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
           if (rx[rsel + uint32_t(st)] <= x) rsel += uint32_t(st);
         x -= rx[rsel];
         const uint32_t j = uint32_t(kReach) + wsel * 16u + rsel;
+        TPC_ASSERT(wsel * 16u + rsel < ncore);
         const uint32_t* r = fw + j * nfw;
         uint32_t bits = 0, wbit = 0;
         bool found = false;
@@ -597,7 +603,9 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
           }
         }
         for (; x; --x) bits &= bits - 1u;                               // drop the x lowest flags
+        TPC_ASSERT(found && bits != 0u);
         const uint32_t pad = wbit + uint32_t(__ffs(bits)) - 1u - uint32_t(kColOff);
+        TPC_ASSERT(pad < ri.npads && map[j * W + pad + kColOff] >= P.theta);
         uint4 lo4, hi4;
         build1(map, fw, W, nfw, j, pad, reinterpret_cast<const uint4*>(nbr_tab), wtab, sector_row, ri.npads, t_row0, P.tf_time_bins,
                lo4, hi4);

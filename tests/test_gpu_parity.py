@@ -572,3 +572,17 @@ def test_two_contexts_with_different_geometries_coexist():
     ref_s, _ = oracle.run(ds, os_, small_np, n_sectors=1, tf_time_bins=50)
     assert got_b.tobytes() == ref_b.tobytes() == got_b2.tobytes() and len(ref_b) > 50
     assert got_s.tobytes() == ref_s.tobytes() and len(ref_s) > 5
+
+
+def test_checked_build_runs_clean():
+    """The -DTPCCLUS_CHECKED build (device asserts on every shared-memory / list index of k_bin and k_tile; the
+    repo's stand-in for compute-sanitizer memcheck, which is closed on this GPU pool) runs the sanitizer cases —
+    smoke, C0, dense C4, time-sorted input, the direct binning kernel, a fragmented TF — without tripping an
+    assert and with records identical to the oracle's."""
+    import subprocess
+    import sys
+
+    p = subprocess.run([sys.executable, os.path.join(HERE, "sanitizer_cases.py"), "--checked"], capture_output=True,
+                       text=True, timeout=900)
+    assert p.returncode == 0, (p.stdout[-1500:], p.stderr[-1500:])
+    assert "sanitizer cases done" in p.stdout
