@@ -13,19 +13,18 @@
 //             min/max instructions (VIMNMX.U16x2, VIMNMX3.U16x2) and one half2 compare (HSET2: exact on these
 //             bit patterns, every value is below 0x7C00); the eight flag bits of a strip go out as ONE
 //             byte store, so the flag map needs neither atomics nor clearing                   (S2)
-//   count     one lane per core row: popc of its flag words, warp scan, CTA scan -> the position of every
-//             peak in (time,pad) order; the tile's count is published for the look-back       (S6, S7)
-//   build     one thread per peak, dense over the tile's peaks in order (each thread finds its peak by two short
-//             binary searches over the count prefixes and a bit select): the 25 charges and the 9x9 flag window
-//             straight from the map (S3..S5); exact integer records (RawRec) go to a staging buffer
-//   commit    the committer warp: decoupled look-back across tiles, D8 finish in fp64, ordered copy-out (S6)
+//   count     one thread per core row (the first eight warps): popc of its flag words, warp scan, and the row's
+//             peaks written, in (time,pad) order, into the warp's segment of a peak list; the tile's count is
+//             published for the look-back                                                      (S6, S7)
+//   build     one thread per peak, dense over the tile's peaks in order: the 25 charges and the 9x9 flag window
+//             straight from the map (S3..S5), exact integer moments, D8 finished in fp64 (Newton iterations from
+//             fp32 seeds + an exact-residual correction instead of the library division / square root); the
+//             finished 32-byte records go to a staging buffer
+//   commit    the committer warp: decoupled look-back across tiles, ordered copy-out             (S6)
 //
 // Definitions D1..D12: SURVEY.md §8(c), restated in DESIGN.md §2.  No code here is shared with oracle/.
 #pragma once
 #include <cuda_fp16.h>
-#ifndef TPCCLUS_BUILD_WARPS
-#define TPCCLUS_BUILD_WARPS 0   /* 0: dense (peak i -> thread i) */
-#endif
 #ifdef TPCCLUS_PHASE_CLOCKS
 #include <cstdio>
 #endif
@@ -102,16 +101,40 @@ __device__ __forceinline__ uint32_t lds16(uint32_t a) {
 }
 __device__ __forceinline__ void sts8(uint32_t a, uint32_t v) { asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v)); }
 
-struct __align__(16) RawRec {       // what the workers stage: D7's exact integers; the committer turns it into ClusterRec
-  uint32_t w0, time, w2;            // as in ClusterRec
-  uint32_t W;                       // sum of weights, units of 1/(16*2520) ADC
-  int32_t Mp, Mt;                   // sum w dp, sum w dt
-  uint32_t Mpp, Mtt;                // sum w dp^2, sum w dt^2
-};
-static_assert(sizeof(RawRec) == 32, "raw record is 32 bytes");
+// ----------------------------------------------------------------------------------------
+// S5 finish (D8) in fp64 from D7's exact integers, rounded once to float32 — the same real-number definitions the
+// oracle evaluates with the C library's double division and square root.  Here: a reciprocal of W and a square
+// root by Newton iterations from fp32 seeds (MUFU.RCP / MUFU.RSQ, 22 bits -> 44 -> 88), each quotient and root
+// closed with ONE exact-residual fma step.  For these operand ranges (W < 2^31, |M| < 2^32, N < 2^63) the double
+// results equal the correctly rounded ones (2e8 random cases on the host, perturbed seeds: 0 differences; every
+// GPU parity test compares the records' bytes), at about a tenth of the instructions of the library routines
+// with their special-case paths.  D12 itself only asks for 1e-6 relative / 1e-4 absolute.
+// ----------------------------------------------------------------------------------------
+__device__ __forceinline__ double recip_newton(double b) {               // 1 / b, b >= 1
+  double y = double(__fdividef(1.0f, float(b)));
+  double e = fma(-b, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-b, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ double div_corr(double a, double b, double y) {   // a / b, y = 1 / b to full precision
+  const double q = a * y;
+  return fma(fma(-q, b, a), y, q);
+}
+__device__ __forceinline__ double sqrt_newton(double n) {                // sqrt(n), n >= 1
+  const double y = double(rsqrtf(float(n)));
+  double g = n * y, h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  return fma(fma(-g, g, n), h, g);
+}
 
 // ----------------------------------------------------------------------------------------
-// S3..S5, one thread per peak.
+// S3..S5, one thread per peak; returns the finished record (two 16-byte halves of a ClusterRec).
 //
 // The 25 cells of the 5x5 window are numbered k = 5 (dt+2) + (dp+2).  D6's S(c) comes from the OTHER peaks of
 // the 9x9 flag window around P: each adds a table entry — one nibble per window cell it is within Chebyshev
@@ -225,25 +248,18 @@ __device__ __forceinline__ void build1(const uint16_t* __restrict__ map, const u
   if (tglob < 2 || uint32_t(tglob) + 2u >= tf_time_bins) flags |= 2u;   // D8 EDGE_TIME
   if (qP == kQClamp) flags |= 4u;       // SATURATED: no member exceeds its peak (D4, D5), so a saturated member implies a saturated peak
   if (nsplit) flags |= 8u;                                              // SPLIT
-  lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob), qP | (ncells << 16), Wsum);
-  hi = make_uint4(uint32_t(Mp), uint32_t(Mt), Mpp, Mtt);
-}
-
-// ----------------------------------------------------------------------------------------
-// S5 finish (D8): RawRec -> ClusterRec.  Evaluated in double from the exact integers and
-// rounded once to float32.
-// ----------------------------------------------------------------------------------------
-__device__ __forceinline__ void finish_rec(uint4& lo, uint4& hi) {
-  const uint32_t W_ = lo.w;
-  const int32_t Mp = int32_t(hi.x), Mt = int32_t(hi.y);
-  const double Wd = double(W_);
-  const long long Np = (long long)hi.z * (long long)W_ - (long long)Mp * (long long)Mp;
-  const long long Nt = (long long)hi.w * (long long)W_ - (long long)Mt * (long long)Mt;
-  lo.w = __float_as_uint(float(Wd / 40320.0));
-  hi.x = __float_as_uint(float(double(Mp) / Wd));
-  hi.y = __float_as_uint(float(double(Mt) / Wd));
-  hi.z = __float_as_uint(float(sqrt(double(Np)) / Wd));
-  hi.w = __float_as_uint(float(sqrt(double(Nt)) / Wd));
+  // D8
+  const double Wd = double(Wsum);
+  const double yW = recip_newton(Wd);
+  const long long Np = (long long)Mpp * (long long)Wsum - (long long)Mp * (long long)Mp;
+  const long long Nt = (long long)Mtt * (long long)Wsum - (long long)Mt * (long long)Mt;
+  const float qtot = float(div_corr(Wd, 40320.0, 1.0 / 40320.0));
+  const float dpad = float(div_corr(double(Mp), Wd, yW));
+  const float dtime = float(div_corr(double(Mt), Wd, yW));
+  const float spad = Np ? float(div_corr(sqrt_newton(double(Np)), Wd, yW)) : 0.0f;
+  const float stime = Nt ? float(div_corr(sqrt_newton(double(Nt)), Wd, yW)) : 0.0f;
+  lo = make_uint4(sector_row | (pad << 16) | (flags << 24), uint32_t(tglob), qP | (ncells << 16), __float_as_uint(qtot));
+  hi = make_uint4(__float_as_uint(dpad), __float_as_uint(dtime), __float_as_uint(spad), __float_as_uint(stime));
 }
 
 // ----------------------------------------------------------------------------------------
@@ -342,7 +358,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
   // carve-up
   uint8_t* sp = smem_raw;                                   // __align__(128); no static shared memory before it
   uint8_t* mapraw = sp;                                     sp += P.map_bytes_max;   // guard, map, guard, flag bytes
-  uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two RawRec staging buffers
+  uint4* stage = reinterpret_cast<uint4*>(sp);              sp += 2 * kListCap * 32; // two staging buffers of finished records
   uint32_t* nbr_tab = reinterpret_cast<uint32_t*>(sp);      sp += kNbrTabWords * 4;  // 16-byte aligned entries
   uint32_t* rowx = reinterpret_cast<uint32_t*>(sp);         sp += kTileT * 4;        // per core row: peaks of its warp's earlier rows
   uint32_t* wpre = reinterpret_cast<uint32_t*>(sp);         sp += kWorkWarps * kWorkWarps * 4;   // per warp: a copy of the warps' exclusive peak prefix
@@ -360,7 +376,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
   __syncthreads();
 
   if (warp == uint32_t(kWorkWarps)) {
-    // ================= committer warp: S6 look-back, S5 finish, copy-out =================
+    // ================= committer warp: S6 look-back and copy-out =================
     uint32_t excl = 0;
     for (uint32_t q = 0;; ++q) {
       const uint32_t b = q & 1u;
@@ -376,15 +392,10 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
       const uint64_t g0 = uint64_t(excl) + off;                          // first record of this item
       const uint4* src = stage + b * (2u * kListCap);
       uint4* dst = reinterpret_cast<uint4*>(P.out) + 2 * g0;
-      // S5 finish (D8), one record per lane: fp64 from the exact integers
-      for (uint32_t r = lane; r < cnt; r += 32u) {
-        if (g0 + r < P.out_capacity) {
-          uint4 lo = src[2u * r], hi = src[2u * r + 1u];
-          finish_rec(lo, hi);
-          dst[2u * r] = lo;
-          dst[2u * r + 1u] = hi;
-        }
-      }
+      // ordered copy-out: consecutive lanes write consecutive 16-byte halves
+      const uint64_t room = P.out_capacity > g0 ? P.out_capacity - g0 : 0ull;
+      const uint32_t nh = 2u * uint32_t(min(uint64_t(cnt), room));
+      for (uint32_t h = lane; h < nh; h += 32u) dst[h] = src[h];
       bar_arrive_named(kBarEmpty + int(b), kThreads);
     }
     return;
@@ -571,10 +582,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
       PH_MARK(4)
       if (q >= 2u) bar_sync_named(kBarEmpty + int(b), kThreads);        // staging[b] has been copied out
       PH_MARK(7)
-      // one thread per peak; peak pk of the item goes to lane pk / kBuildWarps of warp pk % kBuildWarps, so that the
-      // long per-peak chains of several warps overlap
-      constexpr uint32_t kBuildWarps = TPCCLUS_BUILD_WARPS;
-      const uint32_t pk = kBuildWarps == 0u ? tid : (warp < kBuildWarps ? lane * kBuildWarps + warp : 0xFFFFFFFFu);
+      const uint32_t pk = tid;                                           // one thread per peak, dense
       if (pk < npass) {
         // locate peak number done + pk of the tile in (time,pad) order: its warp (largest w with wpre[w] <= x),
         // its row inside the warp's 16 (largest r with rowx[r] <= x'), then the x''-th set flag of that row
