@@ -456,6 +456,11 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     TPC_ASSERT(n <= ri.cap && (reinterpret_cast<uintptr_t>(src) & 15u) == 0u && tt < P.tiles_per_row &&
                flag_off + uint32_t(kBoxH) * fpb + uint32_t(kMapGuard) <= P.map_bytes_max);
 
+    // the first two 16-byte loads of this thread's share of the list are issued before the map is zeroed, so that
+    // their latency overlaps the zeroing and the barrier behind it
+    uint4 pre_a = make_uint4(0u, 0u, 0u, 0u), pre_c = pre_a;
+    if (tid < n4) pre_a = __ldg(src4 + tid);
+    if (tid + kWorkThreads < n4) pre_c = __ldg(src4 + tid + kWorkThreads);
     // ---- D2: zero the tile's charge map, the guard behind it and the flag bytes ----
     {
       const uint32_t nz = (flag_off + uint32_t(kBoxH) * fpb + 15u) >> 4;
@@ -477,7 +482,9 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         TPC_ASSERT(d == 0u || (tl < uint32_t(kBoxH) && dig_pad(d) < ri.npads && dig_q(d) >= 1u && dig_q(d) <= kQClamp));
         if (d && tl < uint32_t(kBoxH)) map[tl * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
       };
-      uint32_t i = tid;
+      put(pre_a.x); put(pre_a.y); put(pre_a.z); put(pre_a.w);            // (zero entries are skipped)
+      put(pre_c.x); put(pre_c.y); put(pre_c.z); put(pre_c.w);
+      uint32_t i = tid + 2 * kWorkThreads;
       for (; i + kWorkThreads < n4; i += 2 * kWorkThreads) {
         const uint4 a = __ldg(src4 + i), c = __ldg(src4 + i + kWorkThreads);
         put(a.x); put(a.y); put(a.z); put(a.w);

@@ -586,3 +586,27 @@ def test_checked_build_runs_clean():
                        text=True, timeout=900)
     assert p.returncode == 0, (p.stdout[-1500:], p.stderr[-1500:])
     assert "sanitizer cases done" in p.stdout
+
+
+def test_peak_lattice_denser_than_a_list_segment():
+    """The densest peak pattern D4 allows — a digit on every second pad of every second time bin, all of them
+    peaks — gives k_tile thousands of peaks per tile: many hand-over items per tile, and more peaks per 32 core
+    rows than a count warp's peak-list segment holds (the per-item list path)."""
+    rng = np.random.default_rng(41)
+    npads = [128, 21, 256]
+    cells = []
+    for r, w in enumerate(npads):
+        for t in range(0, 300, 2):
+            for p in range(r % 2, w, 2):
+                cells.append((0, r, p, t, float(rng.integers(64, 16000)) / 16.0))
+    # a second sector: the same lattice thinned out at random, plus neighbours that make some peaks share cells
+    for (s, r, p, t, q) in list(cells):
+        if rng.random() < 0.5:
+            cells.append((1, r, p, t, q))
+            if rng.random() < 0.3 and p + 1 < npads[r]:
+                cells.append((1, r, p + 1, t, 2.5))
+    d, offs = digits_from_cells(cells, n_sectors=2)
+    for theta in (64, 1):
+        got, ref, st = both(d, offs, npads, n_sectors=2, tf_time_bins=300, peak_min_q16=theta)
+        assert len(ref) > 40000 and st["n_digits_dropped"] == 0
+        assert got.tobytes() == ref.tobytes()
