@@ -48,6 +48,7 @@ class _Params(ctypes.Structure):
         ("npads", ctypes.POINTER(ctypes.c_uint16)),
         ("tf_time_bins", ctypes.c_uint32), ("halo_bins", ctypes.c_uint32),
         ("peak_min_q16", ctypes.c_uint16), ("reserved", ctypes.c_uint16),
+        ("t_time_base", ctypes.c_uint32),
     ]
 
 
@@ -99,7 +100,7 @@ def _load():
     return _lib
 
 
-def _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16):
+def _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16, t_time_base=0):
     npads = np.ascontiguousarray(npads, dtype=np.uint16)
     p = _Params()
     p.n_sectors = int(n_sectors)
@@ -108,6 +109,7 @@ def _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16):
     p.tf_time_bins = int(tf_time_bins)
     p.halo_bins = int(halo_bins)
     p.peak_min_q16 = int(peak_min_q16)
+    p.t_time_base = int(t_time_base)
     return p, npads
 
 
@@ -117,10 +119,11 @@ def quantise(charge: float) -> int:
 
 
 def run(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, t_core_begin=0,
-        t_core_end=None, halo_bins=0, peak_min_q16=64, capacity=None):
+        t_core_end=None, halo_bins=0, peak_min_q16=64, capacity=None, t_time_base=0):
     """Cluster one fragment.  Returns (clusters[CLUSTER_DTYPE], stats dict).
 
-    digits: array of DIGIT_DTYPE grouped per sector by sector_offsets[n_sectors+1].
+    digits: array of DIGIT_DTYPE grouped per sector by sector_offsets[n_sectors+1]; a digit's global time
+    bin is t_time_base + digit.time (reading A19: time frames longer than 65536 bins).
     """
     lib = _load()
     digits = np.ascontiguousarray(digits, dtype=DIGIT_DTYPE)
@@ -128,7 +131,7 @@ def run(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, t_core_begin=
     assert offs.shape[0] == n_sectors + 1
     if t_core_end is None:
         t_core_end = tf_time_bins
-    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16)
+    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16, t_time_base)
     st = _Stats()
     if capacity is None:
         # count first, then allocate exactly
@@ -150,14 +153,14 @@ def run(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, t_core_begin=
 
 
 def peak_flags(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, sector, row,
-               t_core_begin=0, t_core_end=None, halo_bins=0, peak_min_q16=64):
+               t_core_begin=0, t_core_end=None, halo_bins=0, peak_min_q16=64, t_time_base=0):
     """D4 flags and the q16 map of one (sector,row): two arrays [ntime_loaded, npads[row]]."""
     lib = _load()
     digits = np.ascontiguousarray(digits, dtype=DIGIT_DTYPE)
     offs = np.ascontiguousarray(sector_offsets, dtype=np.uint64)
     if t_core_end is None:
         t_core_end = tf_time_bins
-    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16)
+    prm, keep = _params(npads, n_sectors, tf_time_bins, halo_bins, peak_min_q16, t_time_base)
     lo = max(0, t_core_begin - halo_bins)
     hi = min(tf_time_bins, t_core_end + halo_bins)
     w = int(keep[row])

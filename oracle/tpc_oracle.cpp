@@ -9,13 +9,14 @@
 // What it follows.  The paper (PAPER.md:110 §4, :142/:150 §4.2) only names TPC clustering;
 // BASELINE.json:north_star names the five steps; SURVEY.md §8(c) D1..D12 fixes every
 // detail and is the definition this file writes out step by step, in that order and
-// notation (readings A1..A17 are listed in DESIGN.md §3).  Each block cites its D-number.
+// notation (readings A1..A19 are listed in DESIGN.md §3).  Each block cites its D-number.
 //
 // Parity pins (tests/test_oracle_pins.py, tests/test_oracle_bruteforce.py,
 // tests/test_oracle_invariants.py): hand-built maps P1..P9 with values worked out by hand
 // in SURVEY.md §8(c), closed-form Gaussian widths (P8), exhaustive 3x3 / 4x4 and random
 // 8x8 maps against an independently written set/path-form checker in Python with exact
-// Fractions (B1, B2), and invariants I1..I9.  No function here is "parity unpinned".
+// Fractions (B1, B2), and invariants I1..I9; the time base of long time frames (A19) by translation and
+// fragment-seam invariance above bin 65536 (tests/test_oracle_timebase.py).  No function here is "parity unpinned".
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC tpc_oracle.cpp -o libtpc_oracle.so
 #include <cmath>
@@ -87,6 +88,8 @@ struct tpc_oracle_params {
                              // needs the oracle to be able to run with halo 4)
   uint16_t peak_min_q16;     // theta_peak (D11)
   uint16_t reserved;
+  uint32_t t_time_base;      // A19: the digit's u16 time field counts from this global time bin,
+                             // global time = t_time_base + digit.time; 0 for time frames of up to 65536 bins
 };
 
 struct tpc_oracle_stats {
@@ -134,11 +137,12 @@ int tpc_oracle_run(const tpc_oracle_params* prm, const Digit* digits, uint64_t n
     for (uint64_t i = offsets[s]; i < offsets[s + 1]; ++i) {
       const Digit& d = digits[i];
       const uint16_t q16 = tpc_oracle_quantise(d.charge);
+      const int64_t tdig = int64_t(prm->t_time_base) + int64_t(d.time);   // A19: global time bin of the digit
       const bool ok = q16 != 0 && d.row < prm->n_rows && d.pad < prm->npads[d.row] &&
-                      int64_t(d.time) >= lo && int64_t(d.time) < hi;
+                      tdig >= lo && tdig < hi;
       if (!ok) { st->n_digits_dropped++; continue; }
       RowMap& m = rows[d.row];
-      const size_t k = m.idx(d.pad, int(int64_t(d.time) - lo));
+      const size_t k = m.idx(d.pad, int(tdig - lo));
       if (m.q[k] != 0) st->n_duplicates++;
       m.q[k] = q16;
       st->sum_q16_loaded += q16;
@@ -247,8 +251,9 @@ int64_t tpc_oracle_peak_flags(const tpc_oracle_params* prm, const Digit* digits,
   for (uint64_t i = offsets[sector]; i < offsets[sector + 1] && i < n; ++i) {
     const Digit& d = digits[i];
     const uint16_t q16 = tpc_oracle_quantise(d.charge);
-    if (q16 == 0 || d.row != row || d.pad >= prm->npads[row] || int64_t(d.time) < lo || int64_t(d.time) >= hi) continue;
-    m.q[m.idx(d.pad, int(int64_t(d.time) - lo))] = q16;
+    const int64_t tdig = int64_t(prm->t_time_base) + int64_t(d.time);     // A19
+    if (q16 == 0 || d.row != row || d.pad >= prm->npads[row] || tdig < lo || tdig >= hi) continue;
+    m.q[m.idx(d.pad, int(tdig - lo))] = q16;
   }
   for (int t = 0; t < m.ntime; ++t)
     for (int p = 0; p < m.npads; ++p) {
