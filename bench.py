@@ -189,7 +189,8 @@ def make_tf(cfg, device, frags=None):
             continue
         d, offs, info = gen.generate_fragment(cfg, f, device=device,
                                               row_chunk=64 if str(device).startswith("cuda") else 16)
-        out.append(dict(f=f, b=b, e=e, digits=d, offs=offs, n=int(d.shape[0]), occ=info["occupancy"]))
+        out.append(dict(f=f, b=b, e=e, base=info["t_time_base"], digits=d, offs=offs, n=int(d.shape[0]),
+                        occ=info["occupancy"]))
     log(f"generated {cfg.name}: {len(out)} fragments, {sum(x['n'] for x in out):,} digits, "
         f"mean occupancy {np.mean([x['occ'] for x in out]):.4f}, {time.time() - t0:.1f} s on {device}")
     return out
@@ -208,7 +209,7 @@ def oracle_sample(cfg, frag, sectors, threads):
         a, b_ = int(offs[s]), int(offs[s + 1])
         rec, st = oracle.run(dn[a:b_], np.array([0, b_ - a], dtype=np.uint64), npads, n_sectors=1,
                              tf_time_bins=cfg.tf_time_bins, t_core_begin=frag["b"], t_core_end=frag["e"],
-                             halo_bins=cfg.halo_bins, peak_min_q16=THETA)
+                             halo_bins=cfg.halo_bins, peak_min_q16=THETA, t_time_base=frag.get("base", 0))
         return s, rec
 
     oracle.build()
@@ -237,7 +238,7 @@ def run_reference(args):
     d, offs, info = _g.generate_fragment(cfg, 0, device=dev, sectors=range(n_s),
                                          row_chunk=64 if dev != "cpu" else 16)
     b, e = cfg.fragments()[0]
-    frag = dict(b=b, e=e, offs=offs, digits_np=_g.as_numpy_digits(d))
+    frag = dict(b=b, e=e, base=info["t_time_base"], offs=offs, digits_np=_g.as_numpy_digits(d))
     times, nd, ncl = [], 0, 0
     for i in range(args.warmup + args.steps):
         dt, nd, res = oracle_sample(cfg, frag, list(range(n_s)), cores)
@@ -285,7 +286,7 @@ def run_ours(args):
                            max_digits=max_n, cuda_device=local)
     # count pass (capacity 0): cluster counts per fragment -> exact output sizing
     for x in tf:
-        T.tpcclus_run(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["b"], x["e"], 0, 0, stream)
+        T.tpcclus_run_based(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["base"], x["b"], x["e"], 0, 0, stream)
     counts = []
     for x in tf:
         st = T.tpcclus_result(ctx, check=False)
@@ -294,12 +295,13 @@ def run_ours(args):
     n_cl = sum(counts)
     starts = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
     out = torch.zeros((max(n_cl, 1), 32), dtype=torch.uint8, device=dev)
-    log(f"{n_dig:,} digits -> {n_cl:,} clusters; context holds {T.tpcclus_device_bytes(ctx) / 1e9:.2f} GB")
+    ctx_bytes = T.tpcclus_device_bytes(ctx)
+    log(f"{n_dig:,} digits -> {n_cl:,} clusters; context holds {ctx_bytes / 1e9:.2f} GB")
 
     def step():
         for i, x in enumerate(tf):
-            T.tpcclus_run(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["b"], x["e"],
-                          out.data_ptr() + int(starts[i]) * 32, counts[i], stream)
+            T.tpcclus_run_based(ctx, x["digits"].data_ptr(), x["n"], x["offs"], x["base"], x["b"], x["e"],
+                                out.data_ptr() + int(starts[i]) * 32, counts[i], stream)
         for i in range(len(tf)):
             st = T.tpcclus_result(ctx)
             assert st["n_clusters"] == counts[i]
@@ -405,7 +407,8 @@ def run_ours(args):
             fx = tf[fi]
             a, b_ = int(fx["offs"][secs[0]]), int(fx["offs"][secs[-1] + 1])
             offs_local = np.asarray(fx["offs"], dtype=np.int64) - a
-            frag = dict(b=fx["b"], e=fx["e"], offs=offs_local, digits_np=gen.as_numpy_digits(fx["digits"][a:b_]))
+            frag = dict(b=fx["b"], e=fx["e"], base=fx["base"], offs=offs_local,
+                        digits_np=gen.as_numpy_digits(fx["digits"][a:b_]))
             if single is None:      # the same oracle on ONE thread, one sector
                 dt1, nd1, _ = oracle_sample(cfg, frag, secs[:1], 1)
                 single = dict(value=nd1 / dt1, unit=UNIT, cores=1, seconds=dt1,
@@ -440,6 +443,7 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "digits_per_step": n_dig, "clusters_per_step": n_cl,
+                   "fragments": nfr, "context_bytes": int(ctx_bytes), "resident_digit_bytes": int(n_dig * 8),
                    "l2": "inputs larger than L2 (digits %.1f GB per step, %.1f GB per fragment)"
                          % (n_dig * 8 / 1e9, n_dig * 8 / nfr / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -469,7 +473,7 @@ def run_e2e(args, cfg, tf, counts, T, local, world):
         h_out = torch.empty((max(n_cl, 1), 32), dtype=torch.uint8, pin_memory=True)
         torch.cuda.synchronize()
         log(f"e2e: pinned {n_dig * 8 / 1e9:.1f} GB of digits + {n_cl * 32 / 1e9:.1f} GB of records on the host in {time.time() - t0:.1f} s")
-        frs = [(h.data_ptr(), x["n"], x["offs"], x["b"], x["e"]) for h, x in zip(hosts, tf)]
+        frs = [(h.data_ptr(), x["n"], x["offs"], x["b"], x["e"], x["base"]) for h, x in zip(hosts, tf)]
         n_e2e = max(1, min(args.steps, 3))
         for _ in range(1):
             st = T.tpcclus_run_tf_host(ctx, frs, h_out.data_ptr(), n_cl)
@@ -494,7 +498,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="3", help="BASELINE.json config index 0..4 (default 3: the full Pb-Pb TF)")
+    ap.add_argument("--config", default="3", help="BASELINE.json config index 0..4 (default 3: the full Pb-Pb TF), or "
+                    "tf32 | tf128 | tf256: the TF-length sweep of PAPER.md:118 (the C3 generator over 32 / 128 / 256 orbits)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

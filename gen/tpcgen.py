@@ -106,6 +106,14 @@ class Config:
     def npads_array(self) -> np.ndarray:
         return geometry_npads(self.n_rows) if self.npads is None else np.asarray(self.npads, dtype=np.uint16)
 
+    def time_base(self, frag: int) -> int:
+        """Global time bin that the u16 time field of fragment `frag`'s digits counts from (DESIGN.md §3 A19):
+        0 for time frames of up to 65536 bins, else the first loaded bin of the fragment."""
+        if self.tf_time_bins <= 65536:
+            return 0
+        b, _ = self.fragments()[frag]
+        return max(0, b - self.halo_bins)
+
     def fragments(self):
         """Cores [b,e): consecutive chunks of core_bins over the TF (C3: 13 x 4096 + 3776)."""
         out, b = [], 0
@@ -128,6 +136,13 @@ def config(i: int | str, **over) -> Config:
         "c2mini": Config("C2-mini", 3, 2, 1024, 1024, 0, model="c2", occ_row0=0.25, occ_rowN=0.05),
         "c3mini": Config("C3-mini", 4, 2, 1500, 512, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
         "c4mini": Config("C4-mini", 5, 2, 768, 768, 0, model="c4", occ_row0=0.35, occ_rowN=0.35),
+        # TF-length sweep (§4: 32 / 128 / 256 orbits): the C3 generator over
+        # 14256 / 57024 / 114048 time bins (3564 bunch crossings per orbit / 8 per bin), 4096-bin fragments, 8-bin halo
+        "tf32": Config("TF-32-orbits", 4, 36, 14256, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
+        "tf128": Config("TF-128-orbits", 4, 36, 57024, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
+        "tf256": Config("TF-256-orbits", 4, 36, 114048, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
+        # a time frame longer than the u16 time field in small: 130 fragments of 512 bins, the 16-bit boundary at a seam
+        "longmini": Config("TF-long-mini", 4, 2, 66560, 512, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
     }
     return replace(table[i], **over)
 
@@ -250,13 +265,16 @@ def generate_fragment(cfg: Config, frag: int = 0, device="cpu", sectors=None, ro
     Returns (digits, offsets, info): digits is a uint8 tensor [n, 8] on `device` holding
     (u8 row, u8 pad, u16 time, f32 charge) records grouped per sector, in hash-random order
     inside each sector slice; offsets is a numpy uint64 [n_sectors+1]; info has the core
-    range, realised occupancy and an FNV-1a checksum of the buffer's first MiB.
+    range, the time base the u16 time field counts from (cfg.time_base(frag); 0 unless the TF
+    is longer than 65536 bins) and the realised occupancy.
     `sectors` restricts generation to a subset (the other slices are empty).
     """
     dev = torch.device(device)
     b, e = cfg.fragments()[frag]
     lo, hi = max(0, b - cfg.halo_bins), min(cfg.tf_time_bins, e + cfg.halo_bins)
     Tl = hi - lo
+    t_base = cfg.time_base(frag)
+    assert 0 <= lo - t_base and hi - t_base <= 65536
     npads = cfg.npads_array()
     P = int(npads.max())
     npads_t = torch.as_tensor(npads.astype(np.int64), device=dev)
@@ -300,7 +318,7 @@ def generate_fragment(cfg: Config, frag: int = 0, device="cpu", sectors=None, ro
                 # G7: 5 % of the digits (hash-selected) saturate at 1023
                 sat = u01(hash64(seed, TAG_SAT, ck)) < 0.05
                 qk = torch.where(sat, torch.full_like(qk, CHARGE_CLAMP_ADC), qk)
-            word = (ri + r0) | (pi << 8) | ((ti + lo) << 16) | (qk.view(torch.int32).to(torch.int64) << 32)
+            word = (ri + r0) | (pi << 8) | ((ti + (lo - t_base)) << 16) | (qk.view(torch.int32).to(torch.int64) << 32)
             recs.append((word, hash64(seed, TAG_ORDER, ck)))
         word = torch.cat([w for w, _ in recs])
         key = torch.cat([k_ for _, k_ in recs])
@@ -311,7 +329,7 @@ def generate_fragment(cfg: Config, frag: int = 0, device="cpu", sectors=None, ro
     words = torch.cat(parts) if parts else torch.zeros(0, dtype=torch.int64, device=dev)
     digits = words.view(torch.uint8).view(-1, 8)
     n = int(words.numel())
-    info = dict(config=cfg.name, fragment=frag, t_core_begin=b, t_core_end=e, t_loaded=(lo, hi),
+    info = dict(config=cfg.name, fragment=frag, t_core_begin=b, t_core_end=e, t_loaded=(lo, hi), t_time_base=t_base,
                 n_digits=n, n_cells=n_cells * len(want),
                 occupancy=(n / (n_cells * len(want))) if n_cells and want else 0.0)
     return digits, np.asarray(offs, dtype=np.uint64), info

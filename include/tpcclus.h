@@ -72,13 +72,16 @@ extern "C" {
 
 #define TPCCLUS_QMAX_Q16   16368u /* 1023 ADC in 1/16 ADC: the clamp of D1 */
 #define TPCCLUS_MAX_NPADS  256u  /* the pad of a digit is a uint8 */
-#define TPCCLUS_MAX_TF_BINS 65536u /* the time of a digit is a uint16 */
+#define TPCCLUS_MAX_TF_BINS 16777216u /* 2^24 bins; a digit's uint16 time counts from the run's time base */
 #define TPCCLUS_MAX_PENDING 64    /* runs that may be enqueued before their tpcclus_result */
 #define TPCCLUS_MIN_HALO   5u     /* D9: a cluster depends on charges within Chebyshev distance 5 */
 
 /* One zero-suppressed digit, 8 bytes (BASELINE.json:configs[0]: "uint8 row, uint8 pad,
- * uint16 time, float32 charge").  time is the GLOBAL time bin inside the TF.  The sector is
- * not in the record: digits arrive grouped per sector (see sector_offsets below). */
+ * uint16 time, float32 charge").  time counts from the run's time base: GLOBAL time bin inside
+ * the TF = t_time_base + time (base 0 in tpcclus_run, so there it IS the global time bin; time
+ * frames longer than 65536 bins — PAPER.md:118 §4 tested up to 256 orbits = 114048 bins — use
+ * tpcclus_run_based with a base per fragment; DESIGN.md §3 A19).  The sector is not in the
+ * record: digits arrive grouped per sector (see sector_offsets below). */
 typedef struct {
   uint8_t  row;
   uint8_t  pad;
@@ -134,6 +137,9 @@ typedef struct {
   uint64_t n;
   const uint64_t* h_sector_offsets; /* HOST [n_sectors+1]                                      */
   uint32_t t_core_begin, t_core_end;
+  uint32_t t_time_base;             /* global time bin that digit.time counts from (0 for TFs
+                                       of up to 65536 bins)                                    */
+  uint32_t reserved_;               /* must be 0                                               */
 } tpcclus_fragment;
 
 typedef struct tpcclus_ctx tpcclus_ctx; /* opaque; owns all device scratch */
@@ -171,6 +177,16 @@ int tpcclus_run(tpcclus_ctx* ctx, const tpcclus_digit* d_digits, uint64_t n,
                 const uint64_t* h_sector_offsets,
                 uint32_t t_core_begin, uint32_t t_core_end,
                 tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
+
+/* tpcclus_run for digits whose time field counts from t_time_base (DESIGN.md §3 A19): a digit's global
+ * time bin is t_time_base + digit.time; t_core_begin / t_core_end and the records' time stay global.
+ * Needed when tf_time_bins > 65536; a fragment's loaded range [b - halo, e + halo) must lie inside
+ * [t_time_base, t_time_base + 65536) to be expressible.  tpcclus_run == tpcclus_run_based with base 0.
+ * Errors as tpcclus_run; ERR_INVALID also when t_time_base > t_core_begin. */
+int tpcclus_run_based(tpcclus_ctx* ctx, const tpcclus_digit* d_digits, uint64_t n,
+                      const uint64_t* h_sector_offsets, uint32_t t_time_base,
+                      uint32_t t_core_begin, uint32_t t_core_end,
+                      tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
 
 /* Wait for the OLDEST unreported run (FIFO) and report it.  Returns stats->status;
  * ERR_INVALID if no run is pending. */

@@ -35,7 +35,7 @@ CLUSTER_DTYPE = np.dtype([
     ("sigma_pad", "<f4"), ("sigma_time", "<f4")])
 assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
 
-EXPORTS = ("tpcclus_create", "tpcclus_run", "tpcclus_result", "tpcclus_run_host", "tpcclus_run_tf_host",
+EXPORTS = ("tpcclus_create", "tpcclus_run", "tpcclus_run_based", "tpcclus_result", "tpcclus_run_host", "tpcclus_run_tf_host",
            "tpcclus_set_profiling", "tpcclus_get_profile", "tpcclus_launch_count", "tpcclus_device_bytes", "tpcclus_destroy", "tpcclus_strerror")
 
 
@@ -57,7 +57,8 @@ class tpcclus_run_stats(ctypes.Structure):
 class tpcclus_fragment(ctypes.Structure):
     _fields_ = [("h_digits", ctypes.c_void_p), ("n", ctypes.c_uint64),
                 ("h_sector_offsets", ctypes.c_void_p),
-                ("t_core_begin", ctypes.c_uint32), ("t_core_end", ctypes.c_uint32)]
+                ("t_core_begin", ctypes.c_uint32), ("t_core_end", ctypes.c_uint32),
+                ("t_time_base", ctypes.c_uint32), ("reserved_", ctypes.c_uint32)]
 
 
 class TpcclusError(RuntimeError):
@@ -93,6 +94,8 @@ def lib():
             L.tpcclus_create.argtypes = [ctypes.POINTER(tpcclus_geometry), ctypes.c_int, ctypes.POINTER(vp)]
             L.tpcclus_run.restype = ctypes.c_int
             L.tpcclus_run.argtypes = [vp, vp, u64, vp, u32, u32, vp, u64, vp]
+            L.tpcclus_run_based.restype = ctypes.c_int
+            L.tpcclus_run_based.argtypes = [vp, vp, u64, vp, u32, u32, u32, vp, u64, vp]
             L.tpcclus_result.restype = ctypes.c_int
             L.tpcclus_result.argtypes = [vp, ctypes.POINTER(tpcclus_run_stats)]
             L.tpcclus_run_host.restype = ctypes.c_int
@@ -153,6 +156,16 @@ def tpcclus_run(ctx, d_digits_ptr, n, sector_offsets, t_core_begin, t_core_end, 
         raise TpcclusError(rc, "tpcclus_run")
 
 
+def tpcclus_run_based(ctx, d_digits_ptr, n, sector_offsets, t_time_base, t_core_begin, t_core_end, d_out_ptr,
+                      out_capacity, cuda_stream=0):
+    """tpcclus_run for digits whose u16 time counts from t_time_base (time frames longer than 65536 bins)."""
+    offs = _offsets(sector_offsets)
+    rc = lib().tpcclus_run_based(ctx, d_digits_ptr, int(n), offs.ctypes.data, int(t_time_base), int(t_core_begin),
+                                 int(t_core_end), d_out_ptr, int(out_capacity), cuda_stream)
+    if rc != TPCCLUS_OK:
+        raise TpcclusError(rc, "tpcclus_run_based")
+
+
 def tpcclus_result(ctx, check=True):
     """Synchronise the run and return its stats dict; raises on error unless check=False."""
     st = tpcclus_run_stats()
@@ -179,15 +192,17 @@ def tpcclus_run_host(ctx, h_digits, sector_offsets, t_core_begin, t_core_end, h_
 
 
 def tpcclus_run_tf_host(ctx, fragments, h_out_ptr, out_capacity, check=True):
-    """fragments: list of (h_digits_ptr, n, offsets ndarray(uint64), b, e); pointers are HOST addresses."""
+    """fragments: list of (h_digits_ptr, n, offsets ndarray(uint64), b, e[, t_time_base]); pointers are HOST addresses."""
     nf = len(fragments)
     arr = (tpcclus_fragment * nf)()
     keep = []
-    for i, (ptr, n, offs, b, e) in enumerate(fragments):
+    for i, fr in enumerate(fragments):
+        ptr, n, offs, b, e = fr[:5]
         o = _offsets(offs)
         keep.append(o)
         arr[i].h_digits, arr[i].n, arr[i].h_sector_offsets = ptr, int(n), o.ctypes.data
         arr[i].t_core_begin, arr[i].t_core_end = int(b), int(e)
+        arr[i].t_time_base, arr[i].reserved_ = (int(fr[5]) if len(fr) > 5 else 0), 0
     stats = (tpcclus_run_stats * nf)()
     rc = lib().tpcclus_run_tf_host(ctx, arr, nf, h_out_ptr, int(out_capacity), stats)
     out = [dict(n_digits_in=s.n_digits_in, n_digits_dropped=s.n_digits_dropped, n_clusters=s.n_clusters,

@@ -278,9 +278,14 @@ int tpcclus_create(const tpcclus_geometry* g, int cuda_device, tpcclus_ctx** out
 
 int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const uint64_t* h_off,
                 uint32_t b, uint32_t e, tpcclus_cluster* d_out, uint64_t cap, void* cuda_stream) {
+  return tpcclus_run_based(c, d_digits, n, h_off, 0u, b, e, d_out, cap, cuda_stream);
+}
+
+int tpcclus_run_based(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const uint64_t* h_off, uint32_t t_base,
+                      uint32_t b, uint32_t e, tpcclus_cluster* d_out, uint64_t cap, void* cuda_stream) {
   if (!c || !h_off || (n && !d_digits) || (cap && !d_out)) return TPCCLUS_ERR_INVALID;
   const tpcclus_geometry& g = c->g;
-  if (!(b < e) || e > g.tf_time_bins || e - b > g.max_core_bins || n > g.max_digits) return TPCCLUS_ERR_INVALID;
+  if (!(b < e) || e > g.tf_time_bins || e - b > g.max_core_bins || n > g.max_digits || t_base > b) return TPCCLUS_ERR_INVALID;
   if ((reinterpret_cast<uintptr_t>(d_digits) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return TPCCLUS_ERR_INVALID;
   if (h_off[0] != 0 || h_off[g.n_sectors] != n) return TPCCLUS_ERR_INVALID;
   for (uint32_t s = 0; s < g.n_sectors; ++s)
@@ -318,6 +323,7 @@ int tpcclus_run(tpcclus_ctx* c, const tpcclus_digit* d_digits, uint64_t n, const
     bp.n = n;
     bp.sec_list_elems = c->sec_list_elems;
     bp.t_core_begin = int32_t(b);
+    bp.t_base = int32_t(t_base);
     bp.t_lo = std::max<int32_t>(0, int32_t(b) - int32_t(g.halo_bins));
     bp.t_hi = int32_t(std::min<uint64_t>(g.tf_time_bins, uint64_t(e) + g.halo_bins));
     bp.n_sectors = g.n_sectors;
@@ -448,7 +454,7 @@ int tpcclus_run_tf_host(tpcclus_ctx* c, const tpcclus_fragment* fr, uint32_t nf,
     const tpcclus_fragment& x = fr[f];
     if (x.n > c->g.max_digits || (x.n && !x.h_digits) || !x.h_sector_offsets) return TPCCLUS_ERR_INVALID;
     if (!(x.t_core_begin < x.t_core_end) || x.t_core_end > c->g.tf_time_bins ||
-        x.t_core_end - x.t_core_begin > c->g.max_core_bins)
+        x.t_core_end - x.t_core_begin > c->g.max_core_bins || x.t_time_base > x.t_core_begin || x.reserved_ != 0)
       return TPCCLUS_ERR_INVALID;
     if (x.h_sector_offsets[0] != 0 || x.h_sector_offsets[c->g.n_sectors] != x.n) return TPCCLUS_ERR_INVALID;
     for (uint32_t s2 = 0; s2 < c->g.n_sectors; ++s2)
@@ -483,8 +489,8 @@ static int run_tf_host_enqueue(tpcclus_ctx* c, const tpcclus_fragment* fr, uint3
     // kernels of fragment f: need its digits, and the slot's output buffer drained (D2H of f-2)
     CK(c, cudaStreamWaitEvent(c->s_run, c->ev_h2d[slot], 0));
     if (f >= 2) CK(c, cudaStreamWaitEvent(c->s_run, c->ev_d2h[slot], 0));
-    int rc = tpcclus_run(c, c->d_stage_digits[slot], fr[f].n, fr[f].h_sector_offsets, fr[f].t_core_begin,
-                         fr[f].t_core_end, c->d_stage_out[slot], c->g.max_clusters, c->s_run);
+    int rc = tpcclus_run_based(c, c->d_stage_digits[slot], fr[f].n, fr[f].h_sector_offsets, fr[f].t_time_base,
+                               fr[f].t_core_begin, fr[f].t_core_end, c->d_stage_out[slot], c->g.max_clusters, c->s_run);
     if (rc != TPCCLUS_OK) {
       stats[f].status = rc;
       return rc;
@@ -524,6 +530,8 @@ int tpcclus_run_host(tpcclus_ctx* c, const tpcclus_digit* h_digits, uint64_t n, 
   f.h_sector_offsets = h_off;
   f.t_core_begin = b;
   f.t_core_end = e;
+  f.t_time_base = 0;
+  f.reserved_ = 0;
   return tpcclus_run_tf_host(c, &f, 1, h_out, cap, stats);
 }
 

@@ -82,6 +82,7 @@ struct BinParams {
   uint64_t sec_list_elems;             // list elements per sector
   int32_t  t_core_begin;               // b
   int32_t  t_lo, t_hi;                 // loaded range [lo,hi) in global time (D1)
+  int32_t  t_base;                     // A19: global time = t_base + the digit's u16 time field
   uint32_t n_sectors, n_rows;
   uint32_t bins_per_row;               // bins per (sector,row) of this run = ceil((e-b)/kBinT)
   uint32_t bins_per_row_max;           // bins laid out per (sector,row)
@@ -229,7 +230,7 @@ __device__ __forceinline__ bool bin_one(uint32_t w0, uint32_t w1, uint64_t idx, 
                                         uint32_t* __restrict__ counts) {
   while (idx >= P.off[sector + 1]) ++sector;     // digits are grouped per sector; rarely iterates
   const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
-  const int32_t time = int32_t(w0 >> 16);
+  const int32_t time = int32_t(w0 >> 16) + P.t_base;              // A19
   const uint32_t q = quantise_q16(__uint_as_float(w1));
   if (q == 0u || row >= P.n_rows || time < P.t_lo || time >= P.t_hi) return false;
   const RowInfo ri = srow[row];
@@ -529,7 +530,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         const uint32_t j = 2u * pi + uint32_t(h);
         if (full_chunk || j - slot_lo < slot_hi - slot_lo) {
           const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
-          const int32_t time = int32_t(w0 >> 16);
+          const int32_t time = int32_t(w0 >> 16) + P.t_base;        // A19
           const uint32_t q = quantise_q16(__uint_as_float(w1));
           const uint32_t last_pad = (r_npads[row >> 2] >> (8u * (row & 3u))) & 0xFFu;   // npads - 1
           if (q == 0u || uint32_t(time - P.t_lo) >= t_span || pad > last_pad || row >= P.n_rows) {

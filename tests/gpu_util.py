@@ -39,7 +39,7 @@ class GpuClusterizer:
     def __exit__(self, *a):
         self.close()
 
-    def run(self, d_digits, offs, b, e, capacity=None, check=True):
+    def run(self, d_digits, offs, b, e, capacity=None, check=True, t_time_base=0):
         """d_digits: uint8 [n,8] CUDA tensor.  capacity None: count first (capacity 0), then
         run again with exactly the required capacity."""
         import torch
@@ -48,12 +48,12 @@ class GpuClusterizer:
         n = int(d_digits.shape[0])
         stream = torch.cuda.current_stream().cuda_stream
         if capacity is None:
-            T.tpcclus_run(self.ctx, d_digits.data_ptr(), n, offs, b, e, 0, 0, stream)
+            T.tpcclus_run_based(self.ctx, d_digits.data_ptr(), n, offs, t_time_base, b, e, 0, 0, stream)
             st = T.tpcclus_result(self.ctx, check=False)
             assert st["status"] in (T.TPCCLUS_OK, T.TPCCLUS_ERR_CAPACITY), st
             capacity = int(st["n_clusters"])
         out = torch.zeros((max(capacity, 1), 32), dtype=torch.uint8, device="cuda")
-        T.tpcclus_run(self.ctx, d_digits.data_ptr(), n, offs, b, e, out.data_ptr(), capacity, stream)
+        T.tpcclus_run_based(self.ctx, d_digits.data_ptr(), n, offs, t_time_base, b, e, out.data_ptr(), capacity, stream)
         st = T.tpcclus_result(self.ctx, check=check)
         k = min(int(st["n_clusters"]), capacity)
         rec = out[:k].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)

@@ -37,7 +37,7 @@ def test_record_layouts_match_header():
 
     assert ctypes.sizeof(T.tpcclus_geometry) == 56
     assert ctypes.sizeof(T.tpcclus_run_stats) == 32
-    assert ctypes.sizeof(T.tpcclus_fragment) == 32
+    assert ctypes.sizeof(T.tpcclus_fragment) == 40
     assert T.CLUSTER_DTYPE.fields["time"][1] == 4 and T.CLUSTER_DTYPE.fields["qtot"][1] == 12
 
 

@@ -610,3 +610,69 @@ def test_peak_lattice_denser_than_a_list_segment():
         got, ref, st = both(d, offs, npads, n_sectors=2, tf_time_bins=300, peak_min_q16=theta)
         assert len(ref) > 40000 and st["n_digits_dropped"] == 0
         assert got.tobytes() == ref.tobytes()
+
+
+def test_time_frame_longer_than_the_u16_time_field():
+    """DESIGN.md §3 A19 / SURVEY.md §8(f) f-3: a 66560-bin time frame (the C3 generator, 2 sectors, 512-bin fragments
+    with an 8-bin halo); the fragments around bin 65536 and the last one, each with its own time base, through
+    tpcclus_run_based and through tpcclus_run_tf_host, against the oracle; the concatenation against a monolithic
+    oracle run across the 16-bit boundary (I7)."""
+    import paper_2412_13755_b200 as T
+
+    cfg = gen.config("longmini")
+    npads = cfg.npads_array()
+    frs = cfg.fragments()
+    assert len(frs) == 130 and frs[128] == (65536, 66048)
+    pick = [126, 127, 128, 129]
+    kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins, halo_bins=cfg.halo_bins)
+    got_all, host_frs, keep = [], [], []
+    with GpuClusterizer(npads, max_core_bins=cfg.core_bins, max_digits=1 << 24, **kw) as g:
+        for f in pick:
+            b, e = frs[f]
+            base = cfg.time_base(f)
+            assert base == b - 8 and base + 65536 > e + 8
+            d, offs, info = gen.generate_fragment(cfg, f, device="cuda")
+            dn = gen.as_numpy_digits(d)
+            got, st = g.run(d, offs, b, e, t_time_base=base)
+            ref, ost = oracle.run(dn, offs, npads, t_core_begin=b, t_core_end=e, t_time_base=base, **kw)
+            assert st["n_digits_dropped"] == ost["n_digits_dropped"] == 0 and len(ref) > 1e4
+            assert got.tobytes() == ref.tobytes(), f
+            got_all.append(got)
+            keep.append(dn)
+            host_frs.append((dn.ctypes.data, len(dn), offs, b, e, base))
+    cat = np.concatenate(got_all)
+    assert (cat["time"] < 65536).any() and (cat["time"] >= 65536).any() and cat["time"].max() >= 66500
+    assert (cat[cat["time"] >= 66558]["flags"] & 2).all()                  # EDGE_TIME at the true TF end only
+    assert not (cat[(cat["time"] < 66558)]["flags"] & 2).any()
+    # the host-staging pipeline with a base per fragment
+    ctx = T.tpcclus_create(npads, max_core_bins=cfg.core_bins, options=T.TPCCLUS_OPT_HOST_STAGING,
+                           max_digits=max(len(k) for k in keep), max_clusters=max(len(x) for x in got_all) + 1, **kw)
+    try:
+        out = np.zeros(len(cat), dtype=T.CLUSTER_DTYPE)
+        T.tpcclus_run_tf_host(ctx, host_frs, out.ctypes.data, len(cat))
+        assert out.tobytes() == cat.tobytes()
+    finally:
+        T.tpcclus_destroy(ctx)
+    # I7 across bin 65536: one monolithic oracle run over the four cores, digits re-based to the first fragment
+    b0, e1 = frs[pick[0]][0], frs[pick[-1]][1]
+    base0 = cfg.time_base(pick[0])
+    parts = []
+    for dn, fr in zip(keep, host_frs):
+        offs_f, base_f = fr[2], fr[5]
+        sec = np.repeat(np.arange(cfg.n_sectors), np.diff(offs_f).astype(np.int64))
+        key = ((sec.astype(np.int64) * 256 + dn["row"]) * 256 + dn["pad"]) * (1 << 20) + dn["time"].astype(np.int64) + base_f
+        parts.append((key, dn["charge"]))
+    key = np.concatenate([k_ for k_, _ in parts])
+    chg = np.concatenate([c_ for _, c_ in parts])
+    key, first = np.unique(key, return_index=True)                      # halo bins are shared by neighbouring fragments
+    chg = chg[first]
+    dm = np.zeros(len(key), dtype=oracle.DIGIT_DTYPE)
+    dm["time"] = (key % (1 << 20)) - base0
+    dm["pad"] = (key >> 20) % 256
+    dm["row"] = (key >> 28) % 256
+    dm["charge"] = chg
+    om = np.searchsorted(key >> 36, np.arange(cfg.n_sectors + 1)).astype(np.uint64)
+    full, _ = oracle.run(dm, om, npads, n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins, t_core_begin=b0,
+                         t_core_end=e1, halo_bins=8, t_time_base=base0)
+    k = np.lexsort((cat["pad"], cat["time"], cat["row"], cat["sector"]))
+    assert cat[k].tobytes() == full.tobytes()
