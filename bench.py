@@ -179,7 +179,21 @@ def measured_peak_gbs():
 # ----------------------------------------------------------------------------------------------
 # workload
 # ----------------------------------------------------------------------------------------------
-def make_tf(cfg, device, frags=None):
+def sort_within_sectors(d, offs, order):
+    """Digit order inside a sector slice is arbitrary; the configs say "random order".  For the
+    sorted-order timings of BASELINE.md §6: re-order every slice by (row,time,pad) or (time,row,pad)."""
+    import torch
+
+    w = d.view(torch.int64).view(-1)
+    row, pad, tim = w & 0xFF, (w >> 8) & 0xFF, (w >> 16) & 0xFFFF
+    key = (row << 24) | (tim << 8) | pad if order == "row_time_pad" else (tim << 16) | (row << 8) | pad
+    sec = torch.repeat_interleave(torch.arange(len(offs) - 1, device=d.device),
+                                  torch.as_tensor(np.diff(offs).astype(np.int64), device=d.device))
+    idx = torch.argsort(key | (sec << 40))
+    return w[idx].view(torch.uint8).view(-1, 8)
+
+
+def make_tf(cfg, device, frags=None, order="shuffled"):
     import gen
 
     out = []
@@ -189,6 +203,8 @@ def make_tf(cfg, device, frags=None):
             continue
         d, offs, info = gen.generate_fragment(cfg, f, device=device,
                                               row_chunk=64 if str(device).startswith("cuda") else 16)
+        if order != "shuffled":
+            d = sort_within_sectors(d, offs, order)
         out.append(dict(f=f, b=b, e=e, base=info["t_time_base"], digits=d, offs=offs, n=int(d.shape[0]),
                         occ=info["occupancy"]))
     log(f"generated {cfg.name}: {len(out)} fragments, {sum(x['n'] for x in out):,} digits, "
@@ -276,7 +292,7 @@ def run_ours(args):
     dev = f"cuda:{local}"
     cfg = gen.config(args.config)
     npads = cfg.npads_array()
-    tf = make_tf(cfg, dev)
+    tf = make_tf(cfg, dev, order=args.digit_order)
     n_dig = sum(x["n"] for x in tf)
     max_n = max(x["n"] for x in tf)
     stream = torch.cuda.current_stream().cuda_stream
@@ -443,7 +459,7 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u16", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "digits_per_step": n_dig, "clusters_per_step": n_cl,
-                   "fragments": nfr, "context_bytes": int(ctx_bytes), "resident_digit_bytes": int(n_dig * 8),
+                   "digit_order": args.digit_order, "fragments": nfr, "context_bytes": int(ctx_bytes), "resident_digit_bytes": int(n_dig * 8),
                    "l2": "inputs larger than L2 (digits %.1f GB per step, %.1f GB per fragment)"
                          % (n_dig * 8 / 1e9, n_dig * 8 / nfr / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -500,6 +516,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="3", help="BASELINE.json config index 0..4 (default 3: the full Pb-Pb TF), or "
                     "tf32 | tf128 | tf256: the TF-length sweep of PAPER.md:118 (the C3 generator over 32 / 128 / 256 orbits)")
+    ap.add_argument("--digit-order", default="shuffled", choices=["shuffled", "row_time_pad", "time_row_pad"],
+                    help="order of the digits inside each sector slice (the configs' 'random order' is the default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
