@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   uint32_t* buf = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 32u;     // 8 entries per bin
   uint32_t* cnt = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // fill count per bin
   uint2* sec = reinterpret_cast<uint2*>(sp);                  sp += uint32_t(kBinSecCap) * 8u;
-  uint8_t* r_lastpad = reinterpret_cast<uint8_t*>(sp);        sp += 256 * 4;       // npads - 1 per row
+  uint32_t* r_npads = reinterpret_cast<uint32_t*>(sp);        sp += 256 * 4;
   uint32_t* r_off = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint32_t* r_cap = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint64_t* mbar = reinterpret_cast<uint64_t*>(sp);           sp += 16;            // one per staging buffer
@@ -361,7 +361,12 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   const uint32_t tid = threadIdx.x;
   for (uint32_t i = tid; i < 256u; i += kBinThreads) {
     const bool in = i < P.n_rows;
-    r_lastpad[i] = in ? uint8_t(rows[i].npads - 1u) : uint8_t(0);
+    if (i < 64u) {                                            // npads - 1 as bytes, four rows per word
+      uint32_t w = 0;
+      for (uint32_t k = 0; k < 4u; ++k)
+        if (4u * i + k < P.n_rows) w |= (uint32_t(rows[4u * i + k].npads) - 1u) << (8u * k);
+      r_npads[i] = w;
+    }
     r_off[i] = in ? rows[i].list_off : 0u;
     r_cap[i] = in ? rows[i].cap : 0u;
   }
@@ -513,7 +518,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     };
     // ---- phase A: quantise (D1), validate, rank.  An entry ranked >= 8 (its bin's buffer is full)
     //      overwrites its digit in the staging area and is remembered in `pend` for phase B2 ----
-    uint32_t pend = 0, secm = 0;
+    uint32_t pend = 0;
     uint2* stage2 = reinterpret_cast<uint2*>(stage4);
 #pragma unroll
     for (int i = 0; i < kBinPer / 2; ++i) {
@@ -527,7 +532,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
           const uint32_t row = w0 & 0xFFu, pad = (w0 >> 8) & 0xFFu;
           const int32_t time = int32_t(w0 >> 16) + P.t_base;        // A19
           const uint32_t q = quantise_q16(__uint_as_float(w1));
-          const uint32_t last_pad = r_lastpad[row];               // npads - 1 (row is a byte: always inside the table)
+          const uint32_t last_pad = (r_npads[row >> 2] >> (8u * (row & 3u))) & 0xFFu;   // npads - 1
           if (q == 0u || uint32_t(time - P.t_lo) >= t_span || pad > last_pad || row >= P.n_rows) {
             ++dropped;
           } else {
@@ -538,30 +543,24 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
               const uint32_t bin = row * bpr + uint32_t(tlo);
               const uint32_t pk = pack_digit(pad, uint32_t(u - (tlo << kBinShift) + kReach), q);
               const uint32_t r = insert(bin, pk);
-              const bool two = thi != tlo;                    // also in the next bin's window
-              if (r >= 8u || two) stage2[j] = make_uint2(pk, bin | (r << 12));
-              if (r >= 8u) pend |= 1u << (2 * i + h);
-              if (two) secm |= 1u << (2 * i + h);
+              if (r >= 8u) {
+                stage2[j] = make_uint2(pk, bin | (r << 12));
+                pend |= 1u << (2 * i + h);
+              }
+              if (thi != tlo) {                               // also in the next bin's window
+                const uint32_t pk2 = pk - (uint32_t(kBinT) << 8);
+                const uint32_t k2 = atomicAdd(nsecp, 1u);
+                TPC_ASSERT(bin + 1u < P.nb && uint32_t(thi) == uint32_t(tlo) + 1u);
+                if (k2 < uint32_t(kBinSecCap)) {
+                  sec[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
+                } else {                                      // second-entry list full: direct path
+                  const uint32_t cap = r_cap[row];
+                  bin_append<1>(seclist, &counts[cbase + bin + 1u], r_off[row] + uint32_t(tlo + 1) * cap, cap, pk2);
+                }
+              }
             }
           }
         }
-      }
-    }
-    // second entries (a digit within 5 bins of a bin seam, ~4 %): done after the six digits, so that the warp runs
-    // this path once or twice per chunk with whichever lanes have one, not once per digit slot for one or two lanes
-    while (secm) {
-      const uint32_t e = __ffs(secm) - 1;
-      secm &= secm - 1;
-      const uint2 v = stage2[2u * ((e >> 1) * kBinThreads + tid) + (e & 1u)];
-      const uint32_t bin2 = (v.y & 0xFFFu) + 1u, pk2 = v.x - (uint32_t(kBinT) << 8);
-      const uint32_t k2 = atomicAdd(nsecp, 1u);
-      TPC_ASSERT(bin2 < P.nb);
-      if (k2 < uint32_t(kBinSecCap)) {
-        sec[k2] = make_uint2(pk2, bin2 | (insert(bin2, pk2) << 12));
-      } else {                                                // second-entry list full: direct path
-        uint32_t row = bin2 / bpr;
-        const uint32_t cap = r_cap[row];
-        bin_append<1>(seclist, &counts[cbase + bin2], r_off[row] + (bin2 - row * bpr) * cap, cap, pk2);
       }
     }
     __syncthreads();                  // every entry is ranked; buffers and counts are complete
