@@ -375,7 +375,7 @@ def run_ours(args):
     dom = max(kern, key=lambda k: kern[k]["ms_per_launch"])
     # ncu counters of the committed capture of THIS workload (a C3 fragment is a C2 fragment: same generator, same
     # size); null when the capture is of another workload, flagged when the kernels have changed since
-    fragment_like = {"C3-PbPb-TF": "C2-PbPb-fragment"}.get(cfg.name, cfg.name)
+    fragment_like = "C2-PbPb-fragment" if cfg.name.startswith(("C3-", "TF-")) else cfg.name
     ncu = ncu_numbers(fragment_like)
     traffic = ncu["dram_bytes_per_launch"].get(dom) if ncu else None
     # secondary, SM-side ceiling: both kernels are bound by instruction issue, not by HBM.
