@@ -104,33 +104,28 @@ __device__ __forceinline__ void sts8(uint32_t a, uint32_t v) { asm volatile("st.
 // ----------------------------------------------------------------------------------------
 // S5 finish (D8) in fp64 from D7's exact integers, rounded once to float32 — the same real-number definitions the
 // oracle evaluates with the C library's double division and square root.  Here: a reciprocal of W and a square
-// root by Newton iterations from fp32 seeds (MUFU.RCP / MUFU.RSQ, 22 bits -> 44 -> 88), each quotient and root
-// closed with ONE exact-residual fma step.  For these operand ranges (W < 2^31, |M| < 2^32, N < 2^63) the double
-// results equal the correctly rounded ones (2e8 random cases on the host, perturbed seeds: 0 differences; every
+// root by ONE Newton step from fp32 seeds (MUFU.RCP / MUFU.RSQ, 22 bits -> 44), each quotient and root closed
+// with one exact-residual fma step (44 -> 88 bits before the rounding).  For these operand ranges (W < 2^31,
+// |M| < 2^32, N < 2^63) the double results equal the correctly rounded ones (3e8 random cases on the host with
+// seeds perturbed by up to 2^-21: 0 differences; every
 // GPU parity test compares the records' bytes), at about a tenth of the instructions of the library routines
 // with their special-case paths.  D12 itself only asks for 1e-6 relative / 1e-4 absolute.
 // ----------------------------------------------------------------------------------------
 __device__ __forceinline__ double recip_newton(double b) {               // 1 / b, b >= 1
-  double y = double(__fdividef(1.0f, float(b)));
-  double e = fma(-b, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-b, y, 1.0);
-  return fma(y, e, y);
+  const double y = double(__fdividef(1.0f, float(b)));                   // 22 bits
+  return fma(y, fma(-b, y, 1.0), y);                                     // 44 bits; div_corr's residual step does the rest
 }
-__device__ __forceinline__ double div_corr(double a, double b, double y) {   // a / b, y = 1 / b to full precision
+__device__ __forceinline__ double div_corr(double a, double b, double y) {   // a / b, y = 1 / b to 44 bits or better
   const double q = a * y;
   return fma(fma(-q, b, a), y, q);
 }
 __device__ __forceinline__ double sqrt_newton(double n) {                // sqrt(n), n >= 1
   const double y = double(rsqrtf(float(n)));
   double g = n * y, h = 0.5 * y;
-  double r = fma(-g, h, 0.5);
+  const double r = fma(-g, h, 0.5);                                      // one coupled step: 22 -> 44 bits
   g = fma(g, r, g);
   h = fma(h, r, h);
-  r = fma(-g, h, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
-  return fma(fma(-g, g, n), h, g);
+  return fma(fma(-g, g, n), h, g);                                       // exact residual: 44 -> 44 bits or better
 }
 
 // ----------------------------------------------------------------------------------------
