@@ -60,6 +60,14 @@ class _Stats(ctypes.Structure):
     ]
 
 
+class _Cuts(ctypes.Structure):
+    _fields_ = [
+        ("min_qtot", ctypes.c_float), ("min_qmax_q16", ctypes.c_uint16), ("min_ncells", ctypes.c_uint16),
+        ("reject_flags", ctypes.c_uint8), ("reject_single_pad", ctypes.c_uint8),
+        ("reject_single_time", ctypes.c_uint8), ("reserved", ctypes.c_uint8),
+    ]
+
+
 _lock = threading.Lock()
 _lib = None
 
@@ -96,6 +104,9 @@ def _load():
                 ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
                 ctypes.c_void_p, ctypes.c_void_p,
             ]
+            lib.tpc_oracle_select.restype = ctypes.c_uint64
+            lib.tpc_oracle_select.argtypes = [ctypes.c_void_p, ctypes.c_uint64, ctypes.POINTER(_Cuts),
+                                              ctypes.c_void_p, ctypes.c_uint64]
             _lib = lib
     return _lib
 
@@ -171,3 +182,17 @@ def peak_flags(digits, sector_offsets, npads, *, n_sectors, tf_time_bins, sector
                                   flags.ctypes.data, q.ctypes.data)
     assert n == hi - lo
     return flags, q
+
+
+def select(clusters, *, min_qtot=0.0, min_qmax_q16=0, min_ncells=0, reject_flags=0, reject_single_pad=False,
+           reject_single_time=False, capacity=None):
+    """D13: order-preserving quality selection over a cluster list.  Returns (kept records, number kept)."""
+    lib = _load()
+    clusters = np.ascontiguousarray(clusters, dtype=CLUSTER_DTYPE)
+    cuts = _Cuts(float(min_qtot), int(min_qmax_q16), int(min_ncells), int(reject_flags),
+                 1 if reject_single_pad else 0, 1 if reject_single_time else 0, 0)
+    cap = len(clusters) if capacity is None else int(capacity)
+    out = np.zeros(cap, dtype=CLUSTER_DTYPE)
+    kept = int(lib.tpc_oracle_select(clusters.ctypes.data, len(clusters), ctypes.byref(cuts),
+                                     out.ctypes.data if cap else None, cap))
+    return out[: min(kept, cap)], kept

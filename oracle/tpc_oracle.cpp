@@ -16,7 +16,8 @@
 // in SURVEY.md §8(c), closed-form Gaussian widths (P8), exhaustive 3x3 / 4x4 and random
 // 8x8 maps against an independently written set/path-form checker in Python with exact
 // Fractions (B1, B2), and invariants I1..I9; the time base of long time frames (A19) by translation and
-// fragment-seam invariance above bin 65536 (tests/test_oracle_timebase.py).  No function here is "parity unpinned".
+// fragment-seam invariance above bin 65536 (tests/test_oracle_timebase.py); the selection D13 by hand-worked
+// records (tests/test_oracle_select.py).  No function here is "parity unpinned".
 //
 // Build: g++ -O2 -std=c++17 -shared -fPIC tpc_oracle.cpp -o libtpc_oracle.so
 #include <cmath>
@@ -268,6 +269,41 @@ int64_t tpc_oracle_peak_flags(const tpc_oracle_params* prm, const Digit* digits,
       if (q_out) q_out[size_t(t) * m.npads + p] = qc;
     }
   return hi - lo;
+}
+
+// D13 (reading A20; SURVEY.md §8(f) f-4 "cluster-quality cuts ... as parameters", "same
+// code ... with appropriate selections and parameters"): an order-preserving selection over a finished cluster
+// list.  A record is KEPT iff
+//   qtot >= min_qtot  and  qmax_q16 >= min_qmax_q16  and  ncells >= min_ncells  and  (flags & reject_flags) == 0
+//   and not (reject_single_pad  and sigma_pad  == 0)      -- all of the cluster's weight in one pad column
+//   and not (reject_single_time and sigma_time == 0)      -- all of it in one time bin
+// (sigma == 0 exactly iff the central second moment Mxx*W - Mx^2 is 0: D8 evaluates it from exact integers).
+struct tpc_oracle_cuts {
+  float    min_qtot;
+  uint16_t min_qmax_q16;
+  uint16_t min_ncells;
+  uint8_t  reject_flags;
+  uint8_t  reject_single_pad;
+  uint8_t  reject_single_time;
+  uint8_t  reserved;
+};
+
+// Returns the number of records kept; the first min(kept, cap) of them are written to out, in input order.
+uint64_t tpc_oracle_select(const Cluster* in, uint64_t n, const tpc_oracle_cuts* cuts, Cluster* out, uint64_t cap) {
+  uint64_t kept = 0;
+  for (uint64_t i = 0; i < n; ++i) {
+    const Cluster& c = in[i];
+    bool keep = c.qtot >= cuts->min_qtot;
+    keep = keep && c.qmax_q16 >= cuts->min_qmax_q16;
+    keep = keep && c.ncells >= cuts->min_ncells;
+    keep = keep && (c.flags & cuts->reject_flags) == 0;
+    keep = keep && !(cuts->reject_single_pad && c.sigma_pad == 0.0f);
+    keep = keep && !(cuts->reject_single_time && c.sigma_time == 0.0f);
+    if (!keep) continue;
+    if (kept < cap && out) out[kept] = c;
+    ++kept;
+  }
+  return kept;
 }
 
 }  // extern "C"
