@@ -444,6 +444,37 @@ def run_ours(args):
                    seconds=t_cpu, single_thread=single)
         parity = dict(checked=parts, records=nrec, sectors_not_bit_identical=int(bad))
 
+    # ---- D13 selection pass over the step's cluster list, an HBM-bound kernel of its own ----
+    select = None
+    if args.select:
+        cuts = dict(min_qtot=8.0, reject_single_pad=True, reject_single_time=True)
+        sel_out = torch.empty_like(out)
+        for _ in range(3):
+            T.tpcclus_select(ctx, out.data_ptr(), n_cl, sel_out.data_ptr(), n_cl, stream, **cuts)
+            kept = T.tpcclus_select_result(ctx)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 10
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            T.tpcclus_select(ctx, out.data_ptr(), n_cl, sel_out.data_ptr(), n_cl, stream, **cuts)
+            T.tpcclus_select_result(ctx)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_sel = e0.elapsed_time(e1) / reps
+        by = 32.0 * n_cl + 32.0 * kept
+        select = dict(cuts=cuts, records=n_cl, kept=kept, ms=ms_sel, alg_bytes=by, achieved_gbs=by / (ms_sel * 1e-3) / 1e9,
+                      frac_of_hbm_peak=by / (ms_sel * 1e-3) / 1e9 / peak,
+                      note="timed with the host wait of tpcclus_select_result inside (one call per repetition)")
+        if not args.no_cpu and world == 1:
+            got = sel_out[: min(kept, 2_000_000)].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)
+            import oracle
+            head = out[: min(n_cl, 8_000_000)].cpu().numpy().view(T.CLUSTER_DTYPE).reshape(-1)
+            want, _ = oracle.select(head, **cuts)
+            m = min(len(want), len(got))
+            select["parity_first_records"] = dict(compared=m, identical=bool(got[:m].tobytes() == want[:m].tobytes()))
+        del sel_out
+
     # ---- end to end through the C-ABI with HOST buffers (H2D + kernels + D2H inside the timing) ----
     e2e = None
     if not args.no_e2e:
@@ -467,6 +498,8 @@ def run_ours(args):
         "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roofline, "cpu_baseline": cpu, "parity_check": parity,
     }
+    if select is not None:
+        line["select"] = select
     print(json.dumps(line), flush=True)
 
 
@@ -518,6 +551,7 @@ def main():
                     "tf32 | tf128 | tf256: the TF-length sweep of PAPER.md:118 (the C3 generator over 32 / 128 / 256 orbits)")
     ap.add_argument("--digit-order", default="shuffled", choices=["shuffled", "row_time_pad", "time_row_pad"],
                     help="order of the digits inside each sector slice (the configs' 'random order' is the default)")
+    ap.add_argument("--select", action="store_true", help="also time tpcclus_select (D13 quality selection) over the step's clusters")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

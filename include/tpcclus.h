@@ -211,6 +211,33 @@ int tpcclus_run_tf_host(tpcclus_ctx* ctx, const tpcclus_fragment* frags, uint32_
                         tpcclus_cluster* h_out, uint64_t out_capacity,
                         tpcclus_run_stats* stats /* HOST [n_frags] */);
 
+/* ---- quality selection (D13; "appropriate selections and parameters") --------
+ * tpcclus_run rejects nothing: one record per peak (D10).  tpcclus_select is a separate, order-preserving pass over
+ * a finished list.  A record is KEPT iff  qtot >= min_qtot  and  qmax_q16 >= min_qmax_q16  and
+ * ncells >= min_ncells  and  (flags & reject_flags) == 0  and not (reject_single_pad and sigma_pad == 0: all of the
+ * cluster's weight in one pad column)  and not (reject_single_time and sigma_time == 0). */
+typedef struct {
+  float    min_qtot;                /* ADC; 0 keeps all                                        */
+  uint16_t min_qmax_q16;            /* 1/16 ADC                                                */
+  uint16_t min_ncells;
+  uint8_t  reject_flags;            /* TPCCLUS_FLAG_* bits that disqualify a cluster           */
+  uint8_t  reject_single_pad;       /* 0 / 1                                                   */
+  uint8_t  reject_single_time;      /* 0 / 1                                                   */
+  uint8_t  reserved_;               /* must be 0                                               */
+} tpcclus_cuts;
+
+/* Enqueue the selection on `cuda_stream`: the kept records of d_in[0..n) go to d_out in the same order.
+ *   d_in, d_out  DEVICE, 16-byte aligned, must not overlap; d_out holds out_capacity records.
+ *   n            < 2^32.
+ * Asynchronous; tpcclus_select_result waits for it and returns the number of records kept (the number REQUIRED:
+ * when it exceeds out_capacity the first out_capacity kept records are in d_out and the status is
+ * TPCCLUS_ERR_CAPACITY).  One selection in flight per context; it uses scratch of its own (allocated on the first
+ * call and whenever n grows — the only allocation outside tpcclus_create), so it may overlap the context's runs.
+ * Errors: ERR_INVALID, ERR_NOMEM, ERR_CUDA. */
+int tpcclus_select(tpcclus_ctx* ctx, const tpcclus_cluster* d_in, uint64_t n, const tpcclus_cuts* cuts,
+                   tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
+int tpcclus_select_result(tpcclus_ctx* ctx, uint64_t* n_kept /* HOST out */);
+
 /* Per-kernel device timing (for the roofline figures of bench.py): while on, every run is
  * bracketed with CUDA events on ITS stream around k_init (S0), k_bin (S1 routing) and k_tile
  * (S1 fill .. S7); tpcclus_result adds the elapsed times up.  set_profiling(1) resets the sums. */

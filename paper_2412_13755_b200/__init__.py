@@ -36,6 +36,7 @@ CLUSTER_DTYPE = np.dtype([
 assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
 
 EXPORTS = ("tpcclus_create", "tpcclus_run", "tpcclus_run_based", "tpcclus_result", "tpcclus_run_host", "tpcclus_run_tf_host",
+           "tpcclus_select", "tpcclus_select_result",
            "tpcclus_set_profiling", "tpcclus_get_profile", "tpcclus_launch_count", "tpcclus_device_bytes", "tpcclus_destroy", "tpcclus_strerror")
 
 
@@ -59,6 +60,12 @@ class tpcclus_fragment(ctypes.Structure):
                 ("h_sector_offsets", ctypes.c_void_p),
                 ("t_core_begin", ctypes.c_uint32), ("t_core_end", ctypes.c_uint32),
                 ("t_time_base", ctypes.c_uint32), ("reserved_", ctypes.c_uint32)]
+
+
+class tpcclus_cuts(ctypes.Structure):
+    _fields_ = [("min_qtot", ctypes.c_float), ("min_qmax_q16", ctypes.c_uint16), ("min_ncells", ctypes.c_uint16),
+                ("reject_flags", ctypes.c_uint8), ("reject_single_pad", ctypes.c_uint8),
+                ("reject_single_time", ctypes.c_uint8), ("reserved_", ctypes.c_uint8)]
 
 
 class TpcclusError(RuntimeError):
@@ -103,6 +110,10 @@ def lib():
             L.tpcclus_run_tf_host.restype = ctypes.c_int
             L.tpcclus_run_tf_host.argtypes = [vp, ctypes.POINTER(tpcclus_fragment), u32, vp, u64,
                                               ctypes.POINTER(tpcclus_run_stats)]
+            L.tpcclus_select.restype = ctypes.c_int
+            L.tpcclus_select.argtypes = [vp, vp, u64, ctypes.POINTER(tpcclus_cuts), vp, u64, vp]
+            L.tpcclus_select_result.restype = ctypes.c_int
+            L.tpcclus_select_result.argtypes = [vp, ctypes.POINTER(u64)]
             L.tpcclus_set_profiling.restype = ctypes.c_int
             L.tpcclus_set_profiling.argtypes = [vp, ctypes.c_int]
             L.tpcclus_get_profile.restype = ctypes.c_int
@@ -210,6 +221,25 @@ def tpcclus_run_tf_host(ctx, fragments, h_out_ptr, out_capacity, check=True):
     if check and rc != TPCCLUS_OK:
         raise TpcclusError(rc, "tpcclus_run_tf_host")
     return out
+
+
+def tpcclus_select(ctx, d_in_ptr, n, d_out_ptr, out_capacity, cuda_stream=0, *, min_qtot=0.0, min_qmax_q16=0,
+                   min_ncells=0, reject_flags=0, reject_single_pad=False, reject_single_time=False):
+    """Asynchronous D13 selection over n DEVICE records; collect the count with tpcclus_select_result."""
+    cuts = tpcclus_cuts(float(min_qtot), int(min_qmax_q16), int(min_ncells), int(reject_flags),
+                        1 if reject_single_pad else 0, 1 if reject_single_time else 0, 0)
+    rc = lib().tpcclus_select(ctx, d_in_ptr, int(n), ctypes.byref(cuts), d_out_ptr, int(out_capacity), cuda_stream)
+    if rc != TPCCLUS_OK:
+        raise TpcclusError(rc, "tpcclus_select")
+
+
+def tpcclus_select_result(ctx, check=True) -> int:
+    """Waits for the selection; returns the number of records kept (the number required)."""
+    k = ctypes.c_uint64()
+    rc = lib().tpcclus_select_result(ctx, ctypes.byref(k))
+    if rc != TPCCLUS_OK and (check or rc != TPCCLUS_ERR_CAPACITY):
+        raise TpcclusError(rc, "tpcclus_select_result")
+    return int(k.value)
 
 
 def tpcclus_set_profiling(ctx, on: bool) -> None:

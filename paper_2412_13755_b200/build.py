@@ -10,7 +10,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(CSRC, "libtpcclus.so")
 LIB_CHECKED = os.path.join(CSRC, "libtpcclus_checked.so")   # -DTPCCLUS_CHECKED: bounds-checking device asserts
 SOURCES = ["tpcclus.cu"]
-DEPS = ["tpcclus.cu", "tpcclus_kernels.cuh", "tpcclus_tile.cuh", os.path.join("..", "..", "include", "tpcclus.h")]
+DEPS = ["tpcclus.cu", "tpcclus_kernels.cuh", "tpcclus_tile.cuh", "tpcclus_select.cuh", os.path.join("..", "..", "include", "tpcclus.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

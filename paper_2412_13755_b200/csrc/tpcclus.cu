@@ -45,6 +45,14 @@ struct tpcclus_ctx {
   RowInfo* d_rows = nullptr;
   unsigned long long* d_tile_state = nullptr;
   DevStatus* d_status = nullptr;
+  // tpcclus_select (D13): scratch of its own
+  unsigned long long* d_sel_state = nullptr;   // look-back words, one per 1024 records
+  uint32_t sel_tiles_cap = 0, sel_epoch = 0;
+  unsigned long long* d_sel_kept = nullptr;    // [0] records kept, [1] (as u32) the tile ticket
+  unsigned long long* h_sel_kept = nullptr;    // pinned
+  cudaEvent_t ev_sel = nullptr;
+  bool sel_pending = false;
+  uint64_t sel_cap = 0;
   // pinned host ring: one status slot per pending run (results are reported in FIFO order)
   DevStatus* h_status = nullptr;
   struct Pending { uint64_t n, cap; };
@@ -125,6 +133,10 @@ void tpcclus_destroy(tpcclus_ctx* c) {
     if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
     for (int k = 0; k <= TPCCLUS_N_KERNELS; ++k) if (c->ev_prof[i][k]) cudaEventDestroy(c->ev_prof[i][k]);
   }
+  if (c->sel_pending && c->ev_sel) cudaEventSynchronize(c->ev_sel);
+  cudaFree(c->d_sel_state); cudaFree(c->d_sel_kept);
+  if (c->h_sel_kept) cudaFreeHost(c->h_sel_kept);
+  if (c->ev_sel) cudaEventDestroy(c->ev_sel);
   cudaFree(c->d_lists); cudaFree(c->d_counts); cudaFree(c->d_rows); cudaFree(c->d_tile_state); cudaFree(c->d_status);
   if (c->h_status) cudaFreeHost(c->h_status);
   for (int i = 0; i < 2; ++i) {
@@ -533,6 +545,75 @@ int tpcclus_run_host(tpcclus_ctx* c, const tpcclus_digit* h_digits, uint64_t n, 
   f.t_time_base = 0;
   f.reserved_ = 0;
   return tpcclus_run_tf_host(c, &f, 1, h_out, cap, stats);
+}
+
+int tpcclus_select(tpcclus_ctx* c, const tpcclus_cluster* d_in, uint64_t n, const tpcclus_cuts* cuts,
+                   tpcclus_cluster* d_out, uint64_t cap, void* cuda_stream) {
+  if (!c || !cuts || (n && !d_in) || (cap && !d_out) || cuts->reserved_ != 0 || n > 0xFFFFFFFFull || c->sel_pending)
+    return TPCCLUS_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_in) & 15u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return TPCCLUS_ERR_INVALID;
+  if (!(cuts->min_qtot == cuts->min_qtot)) return TPCCLUS_ERR_INVALID;          // NaN threshold
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  CK(c, cudaSetDevice(c->device));
+  const uint32_t n_tiles = uint32_t((n + kSelTile - 1) / kSelTile);
+  if (!c->d_sel_kept) {
+    int rc;
+    if ((rc = dev_alloc(c, &c->d_sel_kept, 16)) != TPCCLUS_OK) return rc;
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->h_sel_kept), 16) != cudaSuccess) return TPCCLUS_ERR_NOMEM;
+    if (cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming) != cudaSuccess) return TPCCLUS_ERR_CUDA;
+  }
+  if (n_tiles > c->sel_tiles_cap) {              // grow the look-back scratch (zeroed: epoch 0 is never used)
+    CK(c, cudaStreamSynchronize(st));
+    if (c->d_sel_state) { cudaFree(c->d_sel_state); c->dev_bytes -= uint64_t(c->sel_tiles_cap) * 8; c->d_sel_state = nullptr; }
+    const uint32_t want = std::max<uint32_t>(n_tiles, 1024u);
+    int rc;
+    if ((rc = dev_alloc(c, &c->d_sel_state, uint64_t(want) * 8)) != TPCCLUS_OK) { c->sel_tiles_cap = 0; return rc; }
+    CK(c, cudaMemset(c->d_sel_state, 0, uint64_t(want) * 8));
+    c->sel_tiles_cap = want;
+    c->sel_epoch = 0;
+  }
+  c->sel_epoch = (c->sel_epoch + 1) & 0x3FFFFFFFu;
+  if (c->sel_epoch == 0) {
+    CK(c, cudaMemsetAsync(c->d_sel_state, 0, uint64_t(c->sel_tiles_cap) * 8, st));
+    c->sel_epoch = 1;
+  }
+  CK(c, cudaMemsetAsync(c->d_sel_kept, 0, 16, st));
+  if (n_tiles) {
+    SelectParams sp;
+    sp.in = reinterpret_cast<const uint4*>(d_in);
+    sp.out = reinterpret_cast<uint4*>(d_out);
+    sp.tile_state = c->d_sel_state;
+    sp.n_kept = c->d_sel_kept;
+    sp.ticket = reinterpret_cast<unsigned int*>(c->d_sel_kept + 1);
+    sp.n = n;
+    sp.out_capacity = cap;
+    sp.n_tiles = n_tiles;
+    sp.epoch = c->sel_epoch;
+    sp.min_qtot = cuts->min_qtot;
+    sp.min_qmax_q16 = cuts->min_qmax_q16;
+    sp.min_ncells = cuts->min_ncells;
+    sp.reject_flags = cuts->reject_flags;
+    sp.reject_single_pad = cuts->reject_single_pad ? 1u : 0u;
+    sp.reject_single_time = cuts->reject_single_time ? 1u : 0u;
+    const uint32_t grid = std::min<uint32_t>(n_tiles, uint32_t(c->n_sm) * 8u);   // all resident: the look-back waits on earlier tiles
+    k_select<<<grid, kSelThreads, 0, st>>>(sp);
+    c->launches++;
+    CK(c, cudaGetLastError());
+  }
+  CK(c, cudaMemcpyAsync(c->h_sel_kept, c->d_sel_kept, 8, cudaMemcpyDeviceToHost, st));
+  CK(c, cudaEventRecord(c->ev_sel, st));
+  c->sel_pending = true;
+  c->sel_cap = cap;
+  return TPCCLUS_OK;
+}
+
+int tpcclus_select_result(tpcclus_ctx* c, uint64_t* n_kept) {
+  if (!c || !n_kept || !c->sel_pending) return TPCCLUS_ERR_INVALID;
+  cudaSetDevice(c->device);
+  c->sel_pending = false;
+  if (cudaEventSynchronize(c->ev_sel) != cudaSuccess) return TPCCLUS_ERR_CUDA;
+  *n_kept = *c->h_sel_kept;
+  return *n_kept > c->sel_cap ? TPCCLUS_ERR_CAPACITY : TPCCLUS_OK;
 }
 
 uint64_t tpcclus_launch_count(const tpcclus_ctx* c) { return c ? c->launches : 0; }

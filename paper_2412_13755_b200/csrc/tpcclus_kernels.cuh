@@ -631,3 +631,4 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
 }  // namespace tpcclus
 
 #include "tpcclus_tile.cuh"
+#include "tpcclus_select.cuh"
