@@ -99,6 +99,14 @@ class ClockSampler:
         except Exception:
             self.p = None
 
+    def wait_ready(self, timeout=5.0):
+        """nvidia-smi needs a few hundred ms to produce its first sample: do not start a short timed region before."""
+        if self.p is None:
+            return
+        t_end = time.time() + timeout
+        while time.time() < t_end and os.path.getsize(self.f.name) == 0:
+            time.sleep(0.02)
+
     def stop(self, t0=None, t1=None):
         import datetime
 
@@ -323,6 +331,7 @@ def run_ours(args):
             assert st["n_clusters"] == counts[i]
 
     clocks = ClockSampler(local)              # started before the warm-up so that it is sampling by the timed region
+    clocks.wait_ready()
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
