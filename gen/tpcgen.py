@@ -141,6 +141,8 @@ def config(i: int | str, **over) -> Config:
         "tf32": Config("TF-32-orbits", 4, 36, 14256, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
         "tf128": Config("TF-128-orbits", 4, 36, 57024, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
         "tf256": Config("TF-256-orbits", 4, 36, 114048, 4096, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
+        # pp-like occupancy on the full detector (the C1 model on 36 sectors): the low-occupancy case of SURVEY.md §8(f) f-4
+        "ppfrag": Config("PP-fragment", 2, 36, 4096, 4096, 0, model="c0", signal_occ=0.01),
         # a time frame longer than the u16 time field in small: 130 fragments of 512 bins, the 16-bit boundary at a seam
         "longmini": Config("TF-long-mini", 4, 2, 66560, 512, 8, model="c2", occ_row0=0.25, occ_rowN=0.05),
     }

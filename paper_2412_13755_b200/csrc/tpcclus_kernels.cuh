@@ -66,7 +66,8 @@ struct RowInfo {              // one per pad row (device table), 32 bytes
   uint16_t segL;              // map rows flagged per segment
   uint16_t ntasks;            // ns * number of segments
   uint32_t rcp_ns;            // ceil(2^16 / ns): task / ns = (task * rcp_ns) >> 16 for task < 512 (ns <= 64)
-  uint32_t pad_[2];
+  uint32_t sparse_max;        // k_tile: lists of up to this many entries take the digit-driven (sparse) path; <= 8 * kWorkThreads
+  uint32_t pad_;
 };
 static_assert(sizeof(RowInfo) == 32, "RowInfo is 32 bytes");
 

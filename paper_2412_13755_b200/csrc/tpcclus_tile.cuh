@@ -454,8 +454,14 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     // the first two 16-byte loads of this thread's share of the list are issued before the map is zeroed, so that
     // their latency overlaps the zeroing and the barrier behind it
     uint4 pre_a = make_uint4(0u, 0u, 0u, 0u), pre_c = pre_a;
+    uint32_t pre_tail = 0u;
     if (tid < n4) pre_a = __ldg(src4 + tid);
     if (tid + kWorkThreads < n4) pre_c = __ldg(src4 + tid + kWorkThreads);
+    // A SPARSE tile (few enough entries that every thread holds its share of the list in registers: n <= 8 per
+    // thread, and fewer than the row's sparse_max) is tested digit by digit instead of sweeping the map: the peak
+    // test then costs per DIGIT, not per cell (the low-occupancy, pp-like path that skips the
+    // dense scan; also the upper, emptier pad rows of the Pb-Pb configs).
+    const bool sparse = n <= ri.sparse_max;
     // ---- D2: zero the tile's charge map, the guard behind it and the flag bytes ----
     {
       const uint32_t nz = (flag_off + uint32_t(kBoxH) * fpb + 15u) >> 4;
@@ -489,7 +495,8 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         const uint4 a = __ldg(src4 + i);
         put(a.x); put(a.y); put(a.z); put(a.w);
       }
-      if (tid < (n & 3u)) put(__ldg(src + 4u * n4 + tid));               // k_bin_direct lists: any length
+      pre_tail = tid < (n & 3u) ? __ldg(src + 4u * n4 + tid) : 0u;       // k_bin_direct lists: any length
+      put(pre_tail);
     }
     bar_sync_named(kBarWork, kWorkThreads);
     PH_MARK(1)
@@ -502,6 +509,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
     // tasks = (strip s, row segment g): consecutive lanes take consecutive strips of one segment.  Segment g loads
     // rows jb .. jb + L + 1 and flags rows jb + 1 .. jb + L, jb = min(g L, kBoxH - 2 - L) (the last segment is moved
     // up so that nothing is read past the map; the rows it shares with its neighbour get the same bytes twice).
+    if (!sparse) {
     for (uint32_t task0 = warp * 30u; task0 < ri.ntasks; task0 += uint32_t(kWorkWarps) * 30u) {   // (one pass for the usual rows)
       const uint32_t L = ri.segL, ns = ri.ns;
       const int32_t tsk = int32_t(task0 + lane) - 1;
@@ -529,6 +537,24 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         if (m + 1u < nout) sts8(f, b1);
         f += fpb;
       }
+    }
+    } else {
+      // digit-driven D4: an entry is a peak iff Q >= theta, Q > the four neighbours earlier in (time,pad) order and
+      // Q >= the four later ones (D3).  Rows 0 and kBoxH - 1 of the window never carry flags (as in the sweep).
+      auto test = [&](uint32_t d) {
+        const uint32_t tl = dig_tl(d), qv = dig_q(d);
+        if (d == 0u || qv < P.theta || tl - 1u >= uint32_t(kBoxH) - 2u) return;
+        const uint32_t col = dig_pad(d) + uint32_t(kColOff);
+        const uint32_t a = map_s + 2u * (tl * W + col);
+        const uint32_t up = a - pitch, dn = a + pitch;
+        const uint32_t early = max(max(lds16(up - 2u), lds16(up)), max(lds16(up + 2u), lds16(a - 2u)));
+        const uint32_t late = max(max(lds16(dn - 2u), lds16(dn)), max(lds16(dn + 2u), lds16(a + 2u)));
+        if (qv > early && qv >= late)
+          atomicOr(reinterpret_cast<uint32_t*>(mapraw + kMapGuard + flag_off) + tl * nfw + 1u + (col >> 5), 1u << (col & 31u));
+      };
+      test(pre_a.x); test(pre_a.y); test(pre_a.z); test(pre_a.w);
+      test(pre_c.x); test(pre_c.y); test(pre_c.z); test(pre_c.w);
+      test(pre_tail);
     }
     bar_sync_named(kBarWork, kWorkThreads);   // flags complete
     PH_MARK(2)
