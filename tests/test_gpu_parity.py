@@ -676,3 +676,47 @@ def test_time_frame_longer_than_the_u16_time_field():
                          t_core_end=e1, halo_bins=8, t_time_base=base0)
     k = np.lexsort((cat["pad"], cat["time"], cat["row"], cat["sector"]))
     assert cat[k].tobytes() == full.tobytes()
+
+
+@pytest.mark.parametrize("n_cells", [4095, 4096, 4097, 4100])
+def test_tile_at_the_sparse_dense_boundary(n_cells):
+    """k_tile tests a tile digit by digit when its list has at most 4096 entries (every thread keeps its share in
+    registers) and sweeps the map otherwise.  One tile with exactly 4095 / 4096 / 4097 / 4100 digits through the
+    direct binning kernel (lists of exact length, also lengths that are not a multiple of 4), blobs with ties and
+    saturation so that neighbouring peaks, shared cells and plateaus occur on both paths."""
+    import paper_2412_13755_b200 as T
+
+    rng = np.random.default_rng(n_cells)
+    npads, nt = 100, 256
+    cells = {}
+    while len(cells) < n_cells:
+        pc, tc = int(rng.integers(npads)), int(rng.integers(nt))
+        for _ in range(9):
+            p, t = pc + int(rng.integers(-2, 3)), tc + int(rng.integers(-2, 3))
+            if 0 <= p < npads and 0 <= t < nt and len(cells) < n_cells:
+                q = float(rng.integers(32, 2000)) / 16.0
+                if rng.random() < 0.25:
+                    q = 9.0
+                if rng.random() < 0.03:
+                    q = 1023.0
+                cells[(p, t)] = q
+    d, offs = digits_from_cells([(0, 0, p, t, q) for (p, t), q in cells.items()])
+    assert len(d) == n_cells
+    for opt in (T.TPCCLUS_OPT_BIN_DIRECT, 0):
+        got, st = gpu_clusters(d, offs, [npads], n_sectors=1, tf_time_bins=nt, options=opt)
+        ref, _ = oracle.run(d, offs, [npads], n_sectors=1, tf_time_bins=nt)
+        assert len(ref) > 300 and got.tobytes() == ref.tobytes(), opt
+
+
+def test_sparse_and_dense_tiles_with_direct_lists():
+    """The C2 generator has both kinds of tile (dense low pad rows, sparse upper ones); through k_bin_direct the
+    lists have arbitrary lengths (tail entries outside the 16-byte loads) on both paths."""
+    import paper_2412_13755_b200 as T
+
+    cfg = gen.config("c2mini", tf_time_bins=700, core_bins=700)
+    d, offs, _ = gen.generate_fragment(cfg, 0, device="cuda")
+    dn = gen.as_numpy_digits(d)
+    kw = dict(n_sectors=cfg.n_sectors, tf_time_bins=cfg.tf_time_bins)
+    got, _ = gpu_clusters(dn, offs, cfg.npads_array(), options=T.TPCCLUS_OPT_BIN_DIRECT, **kw)
+    ref, _ = oracle.run(dn, offs, cfg.npads_array(), **kw)
+    assert len(ref) > 1e4 and got.tobytes() == ref.tobytes()
