@@ -483,8 +483,10 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         TPC_ASSERT(d == 0u || (tl < uint32_t(kBoxH) && dig_pad(d) < ri.npads && dig_q(d) >= 1u && dig_q(d) <= kQClamp));
         if (d && tl < uint32_t(kBoxH)) map[tl * W + dig_pad(d) + kColOff] = uint16_t(dig_q(d));   // 0 = padding
       };
-      put(pre_a.x); put(pre_a.y); put(pre_a.z); put(pre_a.w);            // (zero entries are skipped)
-      put(pre_c.x); put(pre_c.y); put(pre_c.z); put(pre_c.w);
+      // (zero entries are skipped; short lists leave whole warps and every thread's second load empty)
+      const bool has_a = (tid & ~31u) < n4, has_c = n4 > uint32_t(kWorkThreads) + (tid & ~31u);   // warp-uniform
+      if (has_a) { put(pre_a.x); put(pre_a.y); put(pre_a.z); put(pre_a.w); }
+      if (has_c) { put(pre_c.x); put(pre_c.y); put(pre_c.z); put(pre_c.w); }
       uint32_t i = tid + 2 * kWorkThreads;
       for (; i + kWorkThreads < n4; i += 2 * kWorkThreads) {
         const uint4 a = __ldg(src4 + i), c = __ldg(src4 + i + kWorkThreads);
@@ -496,7 +498,7 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         put(a.x); put(a.y); put(a.z); put(a.w);
       }
       pre_tail = tid < (n & 3u) ? __ldg(src + 4u * n4 + tid) : 0u;       // k_bin_direct lists: any length
-      put(pre_tail);
+      if (n & 3u) put(pre_tail);
     }
     bar_sync_named(kBarWork, kWorkThreads);
     PH_MARK(1)
@@ -552,9 +554,9 @@ __global__ void __launch_bounds__(kThreads, kTileCtasPerSm) k_tile(const __grid_
         if (qv > early && qv >= late)
           atomicOr(reinterpret_cast<uint32_t*>(mapraw + kMapGuard + flag_off) + tl * nfw + 1u + (col >> 5), 1u << (col & 31u));
       };
-      test(pre_a.x); test(pre_a.y); test(pre_a.z); test(pre_a.w);
-      test(pre_c.x); test(pre_c.y); test(pre_c.z); test(pre_c.w);
-      test(pre_tail);
+      if ((tid & ~31u) < n4) { test(pre_a.x); test(pre_a.y); test(pre_a.z); test(pre_a.w); }
+      if (n4 > uint32_t(kWorkThreads) + (tid & ~31u)) { test(pre_c.x); test(pre_c.y); test(pre_c.z); test(pre_c.w); }
+      if (n & 3u) test(pre_tail);
     }
     bar_sync_named(kBarWork, kWorkThreads);   // flags complete
     PH_MARK(2)
