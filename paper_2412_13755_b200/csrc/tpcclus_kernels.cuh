@@ -322,7 +322,7 @@ constexpr uint32_t kBinFull     = 0xFFFFFFFFu;              // bin has no room (
 
 __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
   const uint32_t nb4 = (nb + 3u) & ~3u;
-  return 2u * uint32_t(kBinChunk) * 8u + nb4 * 32u + nb4 * 4u + nb4 * 4u + nb4 * 4u + nb4 * 2u + uint32_t(kBinSecCap) * 8u +
+  return 2u * uint32_t(kBinChunk) * 8u + nb4 * 32u + nb4 * 4u + nb4 * 4u + nb4 * 4u + nb4 * 2u + 2u * uint32_t(kBinSecCap) * 8u +
          3u * 256u * 4u + 96u + 128u;
 }
 
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   uint2* stage0 = reinterpret_cast<uint2*>(sp);               sp += 2u * uint32_t(kBinChunk) * 8u;   // two TMA destinations
   uint32_t* buf = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 32u;     // 8 entries per bin
   uint32_t* cnt = reinterpret_cast<uint32_t*>(sp);            sp += nb4 * 4u;      // fill count per bin
-  uint2* sec = reinterpret_cast<uint2*>(sp);                  sp += uint32_t(kBinSecCap) * 8u;
+  uint2* sec = reinterpret_cast<uint2*>(sp);                  sp += 2u * uint32_t(kBinSecCap) * 8u;   // second entries, one list per staging buffer
   uint32_t* r_npads = reinterpret_cast<uint32_t*>(sp);        sp += 256 * 4;
   uint32_t* r_off = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
   uint32_t* r_cap = reinterpret_cast<uint32_t*>(sp);          sp += 256 * 4;
@@ -456,6 +456,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
   // (an empty buffer too: the sector is part of the list now and must not keep stale entries)
   auto flush_all = [&](uint32_t s) {
     uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
+    __syncthreads();                                          // phase B2 of the sector's last chunk (any thread) has filled the buffers
     apply_reservations();
 #pragma unroll
     for (int x = 0; x < 4; ++x) {
@@ -490,8 +491,43 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     b_off[x] = r_off[row] + tb * b_cap[x];
   }
   if (k0 < k1) reserve_all(s);
+  // ---- phase B2 of a chunk (entries ranked >= 8: into the reserved sectors, or back into the emptied buffer) is run
+  //      at the START of the next iteration, in front of that chunk's phase A and without a barrier between them:
+  //      B2 only writes buffer slots below the bin's fill count, phase A only takes ranks from the fill count up, and
+  //      the two use different staging buffers and second-entry lists.  The slow, latency-bound B2 of some warps thus
+  //      overlaps the issue-bound phase A of the others, and a chunk costs two barriers instead of three ----
+  uint32_t pend = 0;                                         // this thread's entries of the previous chunk that wait for B2
+  auto phase_b2 = [&](uint32_t bp, uint32_t* seclist) {      // bp: staging buffer of that chunk
+    const uint2* stage2 = reinterpret_cast<const uint2*>(stage0 + bp * uint32_t(kBinChunk));
+    auto place = [&](uint32_t pk, uint32_t y) {
+      const uint32_t bin = y & 0xFFFu, r = y >> 12;
+      const uint32_t nf8 = uint32_t(nfull[bin]) << 3;
+      TPC_ASSERT(bin < P.nb && r >= 8u);
+      if (r >= nf8) {
+        TPC_ASSERT(r - nf8 < 8u);
+        buf[bin * 8u + (r - nf8)] = pk;
+      } else {
+        const uint32_t d = dst[bin];
+        TPC_ASSERT(d == kBinFull || uint64_t(d) + r < P.sec_list_elems);
+        if (d != kBinFull) seclist[d + r] = pk;
+      }
+    };
+    while (pend) {                    // most lanes have none: the loop runs as long as some lane has one
+      const uint32_t e = __ffs(pend) - 1;
+      pend &= pend - 1;
+      const uint2 v = stage2[2u * ((e >> 1) * kBinThreads + tid) + (e & 1u)];
+      place(v.x, v.y);
+    }
+    const uint2* secp = sec + bp * uint32_t(kBinSecCap);
+    const uint32_t nsec = min(s_ctl[bp], uint32_t(kBinSecCap));
+    for (uint32_t i = tid; i < nsec; i += kBinThreads) {
+      const uint2 e = secp[i];
+      if ((e.y >> 12) >= 8u) place(e.x, e.y);
+    }
+  };
   for (uint32_t k = k0; k < k1; ++k) {
     const uint32_t b = (k - k0) & 1u;
+    if (k > k0) phase_b2(b ^ 1u, lists + uint64_t(s) * P.sec_list_elems);   // of chunk k - 1 (still sector s)
     {
       const uint32_t s_new = s_par[4u * b];
       if (s_new != s) {
@@ -500,13 +536,13 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         reserve_all(s);
       }
     }
-    if (tid == 0 && k + 1 < k1) load(k + 1, sector_of(k + 1, s), b ^ 1u);   // lands while this chunk is processed
     const uint32_t slot_lo = s_par[4u * b + 1u], slot_hi = s_par[4u * b + 2u];
     const bool full_chunk = slot_lo == 0u && slot_hi == uint32_t(kBinChunk);   // no sector seam inside: no per-digit check
     const uint32_t cbase = s * P.nb;
     uint32_t* seclist = lists + uint64_t(s) * P.sec_list_elems;
     uint4* stage4 = reinterpret_cast<uint4*>(stage0 + b * uint32_t(kBinChunk));
     uint32_t* nsecp = s_ctl + b;                             // second entries of this chunk
+    uint2* secb = sec + b * uint32_t(kBinSecCap);
     mbar_wait(mbar + b, (parbits >> b) & 1u);
     parbits ^= 1u << b;
 
@@ -519,7 +555,6 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     };
     // ---- phase A: quantise (D1), validate, rank.  An entry ranked >= 8 (its bin's buffer is full)
     //      overwrites its digit in the staging area and is remembered in `pend` for phase B2 ----
-    uint32_t pend = 0;
     uint2* stage2 = reinterpret_cast<uint2*>(stage4);
 #pragma unroll
     for (int i = 0; i < kBinPer / 2; ++i) {
@@ -553,7 +588,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
                 const uint32_t k2 = atomicAdd(nsecp, 1u);
                 TPC_ASSERT(bin + 1u < P.nb && uint32_t(thi) == uint32_t(tlo) + 1u);
                 if (k2 < uint32_t(kBinSecCap)) {
-                  sec[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
+                  secb[k2] = make_uint2(pk2, (bin + 1u) | (insert(bin + 1u, pk2) << 12));
                 } else {                                      // second-entry list full: direct path
                   const uint32_t cap = r_cap[row];
                   bin_append<1>(seclist, &counts[cbase + bin + 1u], r_off[row] + uint32_t(tlo + 1) * cap, cap, pk2);
@@ -564,7 +599,8 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         }
       }
     }
-    __syncthreads();                  // every entry is ranked; buffers and counts are complete
+    __syncthreads();                  // every entry is ranked (and phase B2 of the previous chunk is done): buffers and counts are complete
+    if (tid == 0 && k + 1 < k1) load(k + 1, sector_of(k + 1, s), b ^ 1u);   // that buffer's last readers were the B2 above; lands during B1
 
     // ---- phase B1: bins holding a whole sector: store it into the sector reserved ahead, request the
     //      next reservation (one global atomic per flush, never waited for), keep the remainder ----
@@ -593,38 +629,12 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
         cnt[bin] = n & 7u;            // entries ranked >= 8 * nfull move to the buffer's front in phase B2
       }
     }
-    __syncthreads();
-
-    // ---- phase B2: entries ranked >= 8: into the reserved sectors, or back into the (now empty) buffer ----
-    auto place = [&](uint32_t pk, uint32_t y) {
-      const uint32_t bin = y & 0xFFFu, r = y >> 12;
-      const uint32_t nf8 = uint32_t(nfull[bin]) << 3;
-      TPC_ASSERT(bin < P.nb && r >= 8u);
-      if (r >= nf8) {
-        TPC_ASSERT(r - nf8 < 8u);
-        buf[bin * 8u + (r - nf8)] = pk;
-      } else {
-        const uint32_t d = dst[bin];
-        TPC_ASSERT(d == kBinFull || uint64_t(d) + r < P.sec_list_elems);
-        if (d != kBinFull) seclist[d + r] = pk;
-      }
-    };
-    while (pend) {                    // most lanes have none: the loop runs as long as some lane has one
-      const uint32_t e = __ffs(pend) - 1;
-      pend &= pend - 1;
-      const uint2 v = stage2[2u * ((e >> 1) * kBinThreads + tid) + (e & 1u)];
-      place(v.x, v.y);
-    }
-    {
-      const uint32_t nsec = min(*nsecp, uint32_t(kBinSecCap));
-      for (uint32_t i = tid; i < nsec; i += kBinThreads) {
-        const uint2 e = sec[i];
-        if ((e.y >> 12) >= 8u) place(e.x, e.y);
-      }
-    }
-    __syncthreads();                  // buffers, staging area and lists are reused by the next chunk
+    __syncthreads();                  // full buffers are out, nfull / dst are set for the chunk's phase B2 (run next iteration)
   }
-  if (k0 < k1) flush_all(s);
+  if (k0 < k1) {
+    phase_b2((k1 - 1u - k0) & 1u, lists + uint64_t(s) * P.sec_list_elems);
+    flush_all(s);
+  }
   dropped = __reduce_add_sync(0xffffffffu, dropped);
   if ((tid & 31u) == 0u && dropped) atomicAdd(&status->n_dropped, (unsigned long long)dropped);
 }
