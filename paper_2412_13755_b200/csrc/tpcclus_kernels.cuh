@@ -606,10 +606,16 @@ __global__ void __launch_bounds__(kBinThreads, 1) k_bin(const __grid_constant__ 
     //      next reservation (one global atomic per flush, never waited for), keep the remainder ----
     if (tid == 0) s_ctl[b ^ 1u] = 0u; // the other buffer's counter is idle until the next chunk's phase A
     apply_reservations();             // (issued in the previous chunk's phase B1)
+    uint32_t n4[4];                   // (the four fill counts are loaded before the first flush: independent round trips)
 #pragma unroll
     for (int x = 0; x < 4; ++x) {
       const uint32_t bin = tid + uint32_t(x) * kBinThreads;
-      const uint32_t n = bin < P.nb ? cnt[bin] : 0u;
+      n4[x] = bin < P.nb ? cnt[bin] : 0u;
+    }
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const uint32_t bin = tid + uint32_t(x) * kBinThreads;
+      const uint32_t n = n4[x];
       if (n >= 8u) {
         const uint4 a = *reinterpret_cast<const uint4*>(buf + bin * 8u);
         const uint4 c = *reinterpret_cast<const uint4*>(buf + bin * 8u + 4u);
