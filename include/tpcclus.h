@@ -51,6 +51,9 @@ extern "C" {
                                      bin_occupancy_pct allows (scratch is sized ahead,
                                      with a margin): the run's records are incomplete; create the
                                      context with a larger bin_occupancy_pct                          */
+#define TPCCLUS_ERR_TOO_LARGE -8  /* tpcclus_select_static only: n exceeds
+                                     TPCCLUS_SELECT_STATIC_MAX_RECORDS, the size its fixed scratch
+                                     array is built for; nothing was enqueued                         */
 
 /* ---- cluster flag bits ---------------------------- */
 #define TPCCLUS_FLAG_EDGE_PAD   0x01u /* peak pad < 2 or >= npads[row]-2                      */
@@ -237,6 +240,28 @@ typedef struct {
 int tpcclus_select(tpcclus_ctx* ctx, const tpcclus_cluster* d_in, uint64_t n, const tpcclus_cuts* cuts,
                    tpcclus_cluster* d_out, uint64_t out_capacity, void* cuda_stream);
 int tpcclus_select_result(tpcclus_ctx* ctx, uint64_t* n_kept /* HOST out */);
+
+/* The same selection (D13) for callers that cannot allocate: code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc.  It needs no context and calls no cudaMalloc / cudaFree / cudaMallocHost / event or
+ * stream creation: the look-back words and the tile ticket that tpcclus_select keeps in allocated scratch live in ONE
+ * fixed `static __device__` array inside the library (8 bytes per 1024 records + 256 bytes = 128.25 KB; every GPU that
+ * loads the library holds it until the process exits).  Runs on the CURRENT device, on `cuda_stream`.
+ *   d_in, d_out   DEVICE, 16-byte aligned, must not overlap; d_out holds out_capacity records.
+ *   n             <= TPCCLUS_SELECT_STATIC_MAX_RECORDS, else TPCCLUS_ERR_TOO_LARGE (nothing enqueued).
+ *   d_n_kept      DEVICE, 8-byte aligned, caller-owned: receives the number of records kept (the number REQUIRED: when it
+ *                 exceeds out_capacity the first out_capacity kept records are in d_out); written in stream order,
+ *                 also for n = 0.  The caller reads it back its own way (this call never synchronises).
+ * Asynchronous: enqueues two memset nodes (the part of the array this call uses starts at zero; d_n_kept) and one
+ * kernel, all capturable.  The first call on a device also looks the array's device address up
+ * (cudaGetSymbolAddress, once per device): make one call — n = 0 will do — before starting a capture.
+ * EVERY call on a device shares the array: two calls that overlap on the GPU (different streams without an
+ * ordering between them, or concurrent branches of one graph) race on it and give undefined output; calls ordered
+ * on one stream, or by events, are fine.  Output is byte-identical to tpcclus_select's.
+ * Errors: ERR_INVALID (null / misaligned pointers, NaN threshold, reserved_ != 0), ERR_TOO_LARGE, ERR_CUDA. */
+#define TPCCLUS_SELECT_STATIC_MAX_RECORDS 16777216ull   /* 2^24 records = 512 MB of cluster list */
+int tpcclus_select_static(const tpcclus_cluster* d_in, uint64_t n, const tpcclus_cuts* cuts,
+                          tpcclus_cluster* d_out, uint64_t out_capacity, uint64_t* d_n_kept /* DEVICE out */,
+                          void* cuda_stream);
 
 /* Per-kernel device timing (for the roofline figures of bench.py): while on, every run is
  * bracketed with CUDA events on ITS stream around k_init (S0), k_bin (S1 routing) and k_tile

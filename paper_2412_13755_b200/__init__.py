@@ -23,6 +23,8 @@ TPCCLUS_ERR_DIGIT = -4
 TPCCLUS_ERR_CUDA = -5
 TPCCLUS_ERR_NOMEM = -6
 TPCCLUS_ERR_OCCUPANCY = -7
+TPCCLUS_ERR_TOO_LARGE = -8
+TPCCLUS_SELECT_STATIC_MAX_RECORDS = 1 << 24
 
 TPCCLUS_FLAG_EDGE_PAD, TPCCLUS_FLAG_EDGE_TIME, TPCCLUS_FLAG_SATURATED, TPCCLUS_FLAG_SPLIT = 1, 2, 4, 8
 TPCCLUS_OPT_STRICT_DIGITS, TPCCLUS_OPT_HOST_STAGING, TPCCLUS_OPT_BIN_DIRECT = 1, 2, 4
@@ -36,7 +38,7 @@ CLUSTER_DTYPE = np.dtype([
 assert DIGIT_DTYPE.itemsize == 8 and CLUSTER_DTYPE.itemsize == 32
 
 EXPORTS = ("tpcclus_create", "tpcclus_run", "tpcclus_run_based", "tpcclus_result", "tpcclus_run_host", "tpcclus_run_tf_host",
-           "tpcclus_select", "tpcclus_select_result",
+           "tpcclus_select", "tpcclus_select_result", "tpcclus_select_static",
            "tpcclus_set_profiling", "tpcclus_get_profile", "tpcclus_launch_count", "tpcclus_device_bytes", "tpcclus_destroy", "tpcclus_strerror")
 
 
@@ -112,6 +114,8 @@ def lib():
                                               ctypes.POINTER(tpcclus_run_stats)]
             L.tpcclus_select.restype = ctypes.c_int
             L.tpcclus_select.argtypes = [vp, vp, u64, ctypes.POINTER(tpcclus_cuts), vp, u64, vp]
+            L.tpcclus_select_static.restype = ctypes.c_int
+            L.tpcclus_select_static.argtypes = [vp, u64, ctypes.POINTER(tpcclus_cuts), vp, u64, vp, vp]
             L.tpcclus_select_result.restype = ctypes.c_int
             L.tpcclus_select_result.argtypes = [vp, ctypes.POINTER(u64)]
             L.tpcclus_set_profiling.restype = ctypes.c_int
@@ -231,6 +235,18 @@ def tpcclus_select(ctx, d_in_ptr, n, d_out_ptr, out_capacity, cuda_stream=0, *, 
     rc = lib().tpcclus_select(ctx, d_in_ptr, int(n), ctypes.byref(cuts), d_out_ptr, int(out_capacity), cuda_stream)
     if rc != TPCCLUS_OK:
         raise TpcclusError(rc, "tpcclus_select")
+
+
+def tpcclus_select_static(d_in_ptr, n, d_out_ptr, out_capacity, d_n_kept_ptr, cuda_stream=0, *, min_qtot=0.0, min_qmax_q16=0,
+                          min_ncells=0, reject_flags=0, reject_single_pad=False, reject_single_time=False):
+    """The D13 selection without a context and without any allocation (scratch in a fixed device array inside the
+    library): n <= TPCCLUS_SELECT_STATIC_MAX_RECORDS DEVICE records on the current device; the kept count goes to the
+    8-byte DEVICE word d_n_kept_ptr in stream order.  Calls that overlap on the GPU race (include/tpcclus.h)."""
+    cuts = tpcclus_cuts(float(min_qtot), int(min_qmax_q16), int(min_ncells), int(reject_flags),
+                        1 if reject_single_pad else 0, 1 if reject_single_time else 0, 0)
+    rc = lib().tpcclus_select_static(d_in_ptr, int(n), ctypes.byref(cuts), d_out_ptr, int(out_capacity), d_n_kept_ptr, cuda_stream)
+    if rc != TPCCLUS_OK:
+        raise TpcclusError(rc, "tpcclus_select_static")
 
 
 def tpcclus_select_result(ctx, check=True) -> int:

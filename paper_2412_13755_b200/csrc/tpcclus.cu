@@ -11,12 +11,22 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
 using namespace tpcclus;
 
 constexpr int kRing = TPCCLUS_MAX_PENDING;
+
+// ---- tpcclus_select_static: k_select's scratch in a fixed device array instead of allocated memory ----
+// Layout: word 0 (as u32) = the tile ticket; words 32.. = one decoupled look-back word per 1024-record tile.
+// In host code this NAME is only a handle for cudaGetSymbolAddress (select_static_scratch below), never a device
+// address.  Every device that loads the library holds its own copy (128.25 KB) until the process exits.
+constexpr uint32_t kSelStaticHdr = 32;                                               // 256 bytes
+constexpr uint32_t kSelStaticTiles = uint32_t(TPCCLUS_SELECT_STATIC_MAX_RECORDS / kSelTile);   // 16384
+static_assert(TPCCLUS_SELECT_STATIC_MAX_RECORDS % kSelTile == 0, "whole tiles");
+static __device__ __align__(256) unsigned long long g_sel_static[kSelStaticHdr + kSelStaticTiles];
 
 static_assert(sizeof(tpcclus_digit) == 8, "digit is 8 bytes");
 static_assert(sizeof(tpcclus_cluster) == 32 && sizeof(tpcclus_cluster) == sizeof(ClusterRec), "cluster is 32 bytes");
@@ -94,6 +104,34 @@ inline void debug_check(cudaStream_t, const char*) {}
     if (e__ != cudaSuccess) return TPCCLUS_ERR_CUDA;    \
   } while (0)
 
+// Device address of g_sel_static on the CURRENT device (and its SM count), looked up once per device with that
+// device current.  Allocates nothing.
+cudaError_t select_static_scratch(unsigned long long** ptr, int* n_sm) {
+  constexpr int kMaxDev = 64;
+  struct PerDevice { bool ready = false; unsigned long long* ptr = nullptr; int n_sm = 0; };
+  static PerDevice table[kMaxDev];
+  static std::mutex mu;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(mu);
+  PerDevice& d = table[dev];
+  if (!d.ready) {
+    unsigned long long* p = nullptr;
+    int sms = 0;
+    if ((e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_sel_static)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if (!p || sms < 1) return cudaErrorUnknown;
+    d.ptr = p;
+    d.n_sm = sms;
+    d.ready = true;
+  }
+  *ptr = d.ptr;
+  *n_sm = d.n_sm;
+  return cudaSuccess;
+}
+
 template <typename T>
 int dev_alloc(tpcclus_ctx* c, T** p, uint64_t bytes) {
   cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes ? bytes : 16);
@@ -120,6 +158,7 @@ const char* tpcclus_strerror(int code) {
     case TPCCLUS_ERR_CUDA: return "CUDA error";
     case TPCCLUS_ERR_NOMEM: return "out of memory";
     case TPCCLUS_ERR_OCCUPANCY: return "digit bin overflow (bin_occupancy_pct too small for this input)";
+    case TPCCLUS_ERR_TOO_LARGE: return "more records than tpcclus_select_static's fixed scratch holds (TPCCLUS_SELECT_STATIC_MAX_RECORDS)";
     default: return "unknown status";
   }
 }
@@ -616,6 +655,47 @@ int tpcclus_select_result(tpcclus_ctx* c, uint64_t* n_kept) {
   if (cudaEventSynchronize(c->ev_sel) != cudaSuccess) return TPCCLUS_ERR_CUDA;
   *n_kept = *c->h_sel_kept;
   return *n_kept > c->sel_cap ? TPCCLUS_ERR_CAPACITY : TPCCLUS_OK;
+}
+
+int tpcclus_select_static(const tpcclus_cluster* d_in, uint64_t n, const tpcclus_cuts* cuts, tpcclus_cluster* d_out,
+                          uint64_t cap, uint64_t* d_n_kept, void* cuda_stream) {
+  if (!cuts || !d_n_kept || (n && !d_in) || (cap && !d_out) || cuts->reserved_ != 0) return TPCCLUS_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_in) & 15u) || (reinterpret_cast<uintptr_t>(d_out) & 15u) ||
+      (reinterpret_cast<uintptr_t>(d_n_kept) & 7u))
+    return TPCCLUS_ERR_INVALID;
+  if (!(cuts->min_qtot == cuts->min_qtot)) return TPCCLUS_ERR_INVALID;          // NaN threshold
+  if (n > TPCCLUS_SELECT_STATIC_MAX_RECORDS) return TPCCLUS_ERR_TOO_LARGE;      // the array has no look-back word for more
+  unsigned long long* scratch = nullptr;
+  int n_sm = 0;
+  if (select_static_scratch(&scratch, &n_sm) != cudaSuccess) return TPCCLUS_ERR_CUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const uint32_t n_tiles = uint32_t((n + kSelTile - 1) / kSelTile);
+  // the array keeps the last call's contents: the ticket and the look-back words this call will use start at zero
+  // (epoch 0 = "nothing published"; the call itself always runs as epoch 1)
+  if (cudaMemsetAsync(scratch, 0, (uint64_t(kSelStaticHdr) + n_tiles) * 8, st) != cudaSuccess) return TPCCLUS_ERR_CUDA;
+  if (cudaMemsetAsync(d_n_kept, 0, 8, st) != cudaSuccess) return TPCCLUS_ERR_CUDA;   // n = 0: no kernel writes it
+  if (n_tiles) {
+    SelectParams sp;
+    sp.in = reinterpret_cast<const uint4*>(d_in);
+    sp.out = reinterpret_cast<uint4*>(d_out);
+    sp.tile_state = scratch + kSelStaticHdr;
+    sp.n_kept = reinterpret_cast<unsigned long long*>(d_n_kept);
+    sp.ticket = reinterpret_cast<unsigned int*>(scratch);
+    sp.n = n;
+    sp.out_capacity = cap;
+    sp.n_tiles = n_tiles;
+    sp.epoch = 1u;
+    sp.min_qtot = cuts->min_qtot;
+    sp.min_qmax_q16 = cuts->min_qmax_q16;
+    sp.min_ncells = cuts->min_ncells;
+    sp.reject_flags = cuts->reject_flags;
+    sp.reject_single_pad = cuts->reject_single_pad ? 1u : 0u;
+    sp.reject_single_time = cuts->reject_single_time ? 1u : 0u;
+    const uint32_t grid = std::min<uint32_t>(n_tiles, uint32_t(n_sm) * 8u);   // tiles are taken by ticket: any grid size is safe
+    k_select<<<grid, kSelThreads, 0, st>>>(sp);
+    if (cudaGetLastError() != cudaSuccess) return TPCCLUS_ERR_CUDA;
+  }
+  return TPCCLUS_OK;
 }
 
 uint64_t tpcclus_launch_count(const tpcclus_ctx* c) { return c ? c->launches : 0; }
