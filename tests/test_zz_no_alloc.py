@@ -118,3 +118,41 @@ def test_select_static_rejects_what_it_cannot_hold():
     torch.cuda.synchronize()
     assert word.tolist() == [16, 7]                            # all-zero records pass the default cuts
     assert ctypes.sizeof(T.tpcclus_cuts) == 12
+
+
+def test_select_static_is_capturable_in_a_cuda_graph():
+    """include/tpcclus.h says the call enqueues two memsets and one kernel, "all capturable": capture it once (after the
+    set-up call), replay the graph twice with different inputs in the same buffers, compare with the existing path."""
+    import torch
+    import paper_2412_13755_b200 as T
+
+    g, rec = _records()
+    try:
+        n = len(rec) // 2                                      # two different inputs of the same length
+        assert n > 1e5
+        a = torch.from_numpy(rec[:n].view(np.uint8).reshape(-1, 32).copy()).cuda()
+        b = torch.from_numpy(rec[n: 2 * n].view(np.uint8).reshape(-1, 32).copy()).cuda()
+        cuts = dict(min_qtot=18.0, reject_single_time=True)
+        cur = torch.cuda.current_stream().cuda_stream
+        want = [_existing(T, g.ctx, x, n, n, cur, **cuts) for x in (a, b)]
+        assert want[0][0] != want[1][0] and 0 < want[0][1] < n
+
+        d_in = torch.zeros_like(a)
+        d_out = torch.zeros((n, 32), dtype=torch.uint8, device="cuda")
+        kept = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+        T.tpcclus_select_static(0, 0, 0, 0, kept.data_ptr(), cur)      # once-per-device set-up, outside the capture
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            T.tpcclus_select_static(d_in.data_ptr(), n, d_out.data_ptr(), n, kept.data_ptr(),
+                                    torch.cuda.current_stream().cuda_stream, **cuts)
+        for x, (w_bytes, w_kept) in zip((a, b), want):
+            d_in.copy_(x)
+            d_out.zero_()
+            graph.replay()
+            torch.cuda.synchronize()
+            k = int(kept.item())
+            assert k == w_kept
+            assert d_out[:k].cpu().numpy().tobytes() == w_bytes
+    finally:
+        g.close()
