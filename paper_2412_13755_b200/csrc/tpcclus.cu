@@ -636,6 +636,7 @@ int tpcclus_select(tpcclus_ctx* c, const tpcclus_cluster* d_in, uint64_t n, cons
     sp.reject_flags = cuts->reject_flags;
     sp.reject_single_pad = cuts->reject_single_pad ? 1u : 0u;
     sp.reject_single_time = cuts->reject_single_time ? 1u : 0u;
+    sp.wide = ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_out)) & 31u) == 0u ? 1u : 0u;
     const uint32_t grid = std::min<uint32_t>(n_tiles, uint32_t(c->n_sm) * 8u);   // all resident: the look-back waits on earlier tiles
     k_select<<<grid, kSelThreads, 0, st>>>(sp);
     c->launches++;
@@ -691,6 +692,7 @@ int tpcclus_select_static(const tpcclus_cluster* d_in, uint64_t n, const tpcclus
     sp.reject_flags = cuts->reject_flags;
     sp.reject_single_pad = cuts->reject_single_pad ? 1u : 0u;
     sp.reject_single_time = cuts->reject_single_time ? 1u : 0u;
+    sp.wide = ((reinterpret_cast<uintptr_t>(d_in) | reinterpret_cast<uintptr_t>(d_out)) & 31u) == 0u ? 1u : 0u;
     const uint32_t grid = std::min<uint32_t>(n_tiles, uint32_t(n_sm) * 8u);   // tiles are taken by ticket: any grid size is safe
     k_select<<<grid, kSelThreads, 0, st>>>(sp);
     if (cudaGetLastError() != cudaSuccess) return TPCCLUS_ERR_CUDA;

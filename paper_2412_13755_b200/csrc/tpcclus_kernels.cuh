@@ -330,9 +330,11 @@ __host__ __device__ inline uint32_t bin_smem_bytes(uint32_t nb) {
 // reservations stop being multiples of 8 only after a single-entry append (second entries beyond kBinSecCap,
 // i.e. time-sorted input), and then the entries go out one by one
 __device__ __forceinline__ void store8(uint32_t* p, uint4 a, uint4 c) {
-  if ((reinterpret_cast<uintptr_t>(p) & 15u) == 0u) {
-    *reinterpret_cast<uint4*>(p) = a;
-    *reinterpret_cast<uint4*>(p + 4) = c;
+  if ((reinterpret_cast<uintptr_t>(p) & 31u) == 0u) {
+    // ONE 256-bit store (sm_100): the sector goes through the LSU as one access instead of two
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w),
+                 "r"(c.x), "r"(c.y), "r"(c.z), "r"(c.w)
+                 : "memory");
   } else {
     p[0] = a.x; p[1] = a.y; p[2] = a.z; p[3] = a.w;
     p[4] = c.x; p[5] = c.y; p[6] = c.z; p[7] = c.w;

@@ -20,12 +20,26 @@ struct SelectParams {
   uint32_t n_tiles, epoch;
   float min_qtot;
   uint32_t min_qmax_q16, min_ncells, reject_flags, reject_single_pad, reject_single_time;
+  uint32_t wide;                       // in and out are 32-byte aligned: records move as single 256-bit accesses
 };
 
 constexpr int kSelThreads = 256;
 constexpr int kSelPer = 4;                                   // records per thread
 constexpr int kSelTile = kSelThreads * kSelPer;              // 1024 records = 32 KB
 constexpr int kSelWarps = kSelThreads / 32;
+
+// A 32-byte record as ONE 256-bit access (sm_100: LDG / STG .256): a warp instruction then touches every 128-byte line
+// once, where two 16-byte halves touch it twice — the LSU's line rate, not bytes, is what bounds this kernel.
+__device__ __forceinline__ void ld_rec(const uint4* p, uint4& lo, uint4& hi) {
+  asm volatile("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(lo.x), "=r"(lo.y), "=r"(lo.z), "=r"(lo.w), "=r"(hi.x), "=r"(hi.y), "=r"(hi.z), "=r"(hi.w)
+               : "l"(p));
+}
+__device__ __forceinline__ void st_rec(uint4* p, const uint4& lo, const uint4& hi) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(lo.x), "r"(lo.y), "r"(lo.z), "r"(lo.w),
+               "r"(hi.x), "r"(hi.y), "r"(hi.z), "r"(hi.w)
+               : "memory");
+}
 
 __device__ __forceinline__ bool select_keep(const SelectParams& P, const uint4& lo, const uint4& hi) {
   // ClusterRec: lo = {sector | row << 8 | pad << 16 | flags << 24, time, qmax_q16 | ncells << 16, qtot}, hi = {dpad, dtime, sigma_pad, sigma_time}
@@ -58,8 +72,12 @@ __global__ void __launch_bounds__(kSelThreads) k_select(const __grid_constant__ 
       const uint64_t i = first + uint64_t(k) * kSelThreads;
       bool keep = false;
       if (i < P.n) {
-        lo[k] = __ldg(P.in + 2 * i);                         // (L1-allocating: the two halves of a record share a 32-byte sector)
-        hi[k] = __ldg(P.in + 2 * i + 1);
+        if (P.wide) {
+          ld_rec(P.in + 2 * i, lo[k], hi[k]);
+        } else {                                             // buffers aligned to 16 but not to 32 bytes
+          lo[k] = __ldg(P.in + 2 * i);
+          hi[k] = __ldg(P.in + 2 * i + 1);
+        }
         keep = select_keep(P, lo[k], hi[k]);
       }
       const uint32_t bal = __ballot_sync(0xffffffffu, keep);
@@ -94,8 +112,12 @@ __global__ void __launch_bounds__(kSelThreads) k_select(const __grid_constant__ 
       if (keepm & (1u << k)) {
         const uint64_t pos = base + s_off[k * kSelWarps + warp] + rank[k];
         if (pos < P.out_capacity) {
-          P.out[2 * pos] = lo[k];
-          P.out[2 * pos + 1] = hi[k];
+          if (P.wide) {
+            st_rec(P.out + 2 * pos, lo[k], hi[k]);
+          } else {
+            P.out[2 * pos] = lo[k];
+            P.out[2 * pos + 1] = hi[k];
+          }
         }
       }
     }

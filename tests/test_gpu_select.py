@@ -78,3 +78,45 @@ def test_select_argument_errors():
         assert T.tpcclus_select_result(ctx) == 0
     finally:
         T.tpcclus_destroy(ctx)
+
+
+@pytest.mark.parametrize("in_off,out_off", [(0, 0), (16, 0), (0, 16), (16, 16)])
+def test_select_alignment_classes(in_off, out_off):
+    """Buffers aligned to 32 bytes move records as single 256-bit accesses, buffers aligned to 16 bytes only as two
+    halves (include/tpcclus.h asks for 16): both paths, and their mixes, give the oracle's bytes."""
+    import torch
+    import paper_2412_13755_b200 as T
+
+    rng = np.random.default_rng(7 + in_off + 2 * out_off)
+    n = 5000
+    rec = np.zeros(n, dtype=T.CLUSTER_DTYPE)
+    rec["sector"], rec["row"], rec["pad"] = 0, rng.integers(0, 4, n), rng.integers(0, 100, n)
+    rec["time"] = np.arange(n)
+    rec["flags"] = rng.integers(0, 16, n)
+    rec["qmax_q16"], rec["ncells"] = rng.integers(64, 16368, n), rng.integers(1, 25, n)
+    rec["qtot"] = rng.integers(64, 40000, n) / 16.0
+    rec["sigma_pad"] = np.where(rng.random(n) < 0.2, 0.0, rng.random(n)).astype(np.float32)
+    rec["sigma_time"] = np.where(rng.random(n) < 0.2, 0.0, rng.random(n)).astype(np.float32)
+    cuts = dict(min_qtot=300.0, min_ncells=3, reject_single_pad=True, reject_flags=2)
+    want, kept_o = oracle.select(rec.view(oracle.CLUSTER_DTYPE), **cuts)
+    assert 0 < kept_o < n
+    raw = torch.zeros(n * 32 + 64, dtype=torch.uint8, device="cuda")
+    out = torch.zeros(n * 32 + 64, dtype=torch.uint8, device="cuda")
+    base_in = raw.data_ptr() + (-raw.data_ptr()) % 32 + in_off
+    base_out = out.data_ptr() + (-out.data_ptr()) % 32 + out_off
+    o_in, o_out = base_in - raw.data_ptr(), base_out - out.data_ptr()
+    raw[o_in: o_in + n * 32] = torch.from_numpy(rec.view(np.uint8).copy()).cuda()
+    ctx = T.tpcclus_create([100], n_sectors=1, tf_time_bins=100, max_digits=10)
+    try:
+        T.tpcclus_select(ctx, base_in, n, base_out, n, torch.cuda.current_stream().cuda_stream, **cuts)
+        kept = T.tpcclus_select_result(ctx)
+        assert kept == kept_o
+        assert out[o_out: o_out + kept * 32].cpu().numpy().tobytes() == want.tobytes()
+        word = torch.zeros(1, dtype=torch.int64, device="cuda")
+        out.zero_()
+        T.tpcclus_select_static(base_in, n, base_out, n, word.data_ptr(), torch.cuda.current_stream().cuda_stream, **cuts)
+        torch.cuda.synchronize()
+        assert int(word.item()) == kept_o
+        assert out[o_out: o_out + kept * 32].cpu().numpy().tobytes() == want.tobytes()
+    finally:
+        T.tpcclus_destroy(ctx)
