@@ -77,3 +77,22 @@ def test_product_reads_no_environment_variables():
         for f in files:
             if f.endswith((".cu", ".cuh", ".h")):
                 assert "getenv" not in open(os.path.join(dirpath, f)).read(), f
+
+
+def test_binding_constants_match_the_header():
+    """Every integer `#define TPCCLUS_*` of include/tpcclus.h has the same value in the ctypes binding (error codes,
+    flag and option bits, limits), and every error code has a message of its own."""
+    import paper_2412_13755_b200 as T
+
+    src = open(os.path.join(ROOT, "include", "tpcclus.h")).read()
+    defs = dict(re.findall(r"^#define\s+(TPCCLUS_[A-Z0-9_]+)\s+(-?(?:0x[0-9a-fA-F]+|\d+))(?:u|ull)?\b", src, flags=re.M))
+    assert {"TPCCLUS_OK", "TPCCLUS_ERR_CAPACITY", "TPCCLUS_ERR_TOO_LARGE", "TPCCLUS_OPT_BIN_DIRECT",
+            "TPCCLUS_SELECT_STATIC_MAX_RECORDS", "TPCCLUS_FLAG_SPLIT"} <= set(defs)
+    missing = [n for n in defs if not hasattr(T, n) and not n.endswith("_H")]
+    # limits that only the C side needs may be absent from the binding; codes, flags and options may not
+    assert not [n for n in missing if n.startswith(("TPCCLUS_ERR_", "TPCCLUS_FLAG_", "TPCCLUS_OPT_"))], missing
+    for name, text in defs.items():
+        if hasattr(T, name):
+            assert getattr(T, name) == int(text, 0), name
+    msgs = {T.tpcclus_strerror(int(v, 0)) for n, v in defs.items() if n.startswith("TPCCLUS_ERR_")}
+    assert len(msgs) == len([n for n in defs if n.startswith("TPCCLUS_ERR_")]) and "unknown status" not in msgs
